@@ -1,0 +1,276 @@
+"""Seeded synthetic workloads (inputs only — none of the method's arithmetic lives here).
+
+Both the CPU oracle (oracle/) and the CUDA library are fed from this module; it imports
+neither.  The five workloads stand in for the paper's inputs, which are not available
+(C5G7-TD cross sections and pin map; MC/DC's continuous-energy library and
+examples/fixed_source/inf_pin_ce/input.py).  They take the *shape* of those
+workloads as BASELINE.json configs[0..4] describe them; the recipe is stated in DESIGN.md
+section 4.  Problem seed 0x25060263 (numpy PCG64), run seed 1.
+"""
+from __future__ import annotations
+
+from dataclasses import dataclass, field
+from typing import Optional
+
+import numpy as np
+
+MAX_RINGS = 4
+MAX_NUC = 4
+PROBLEM_SEED = 0x25060263
+INF = float("inf")
+
+
+@dataclass
+class Problem:
+    name: str
+    geometry: dict
+    materials: dict
+    xs: Optional[dict]
+    mode: str                       # "fixed" | "k"
+    n_particles: int
+    n_inactive: int = 0
+    n_active: int = 0
+    seed: int = 1
+    notes: dict = field(default_factory=dict)
+
+
+def _f64(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.float64))
+
+
+def _i32(a):
+    return np.ascontiguousarray(np.asarray(a, dtype=np.int32))
+
+
+def geometry(xplanes, yplanes, zplanes, cell_univ, universes, bc, mesh=None, by_group=0,
+             e_edges=None, src_kind=0, src_lo=(0, 0, 0), src_hi=(0, 0, 0), src_dir=None,
+             src_energy=("group", 0), scale_log2=24, cx=None, cy=None):
+    """universes: list of (radii ascending, materials innermost..background)."""
+    xp, yp, zp = _f64(xplanes), _f64(yplanes), _f64(zplanes)
+    nx, ny, nz = len(xp) - 1, len(yp) - 1, len(zp) - 1
+    if cx is None:
+        cx = [0.5 * (xp[i] + xp[i + 1]) if np.isfinite(xp[i]) and np.isfinite(xp[i + 1]) else 0.0 for i in range(nx)]
+    if cy is None:
+        cy = [0.5 * (yp[i] + yp[i + 1]) if np.isfinite(yp[i]) and np.isfinite(yp[i + 1]) else 0.0 for i in range(ny)]
+    nr = _i32([len(u[0]) for u in universes])
+    rad = np.zeros((len(universes), MAX_RINGS))
+    mat = np.zeros((len(universes), MAX_RINGS + 1), dtype=np.int32)
+    for k, (radii, mats) in enumerate(universes):
+        assert len(mats) == len(radii) + 1 and len(radii) <= MAX_RINGS
+        rad[k, :len(radii)] = radii
+        mat[k, :len(mats)] = mats
+    if mesh is None:
+        mesh = ([xp[0], xp[-1]], [yp[0], yp[-1]], [zp[0], zp[-1]])
+    ekind = {"group": 0, "mono": 1, "watt": 2}[src_energy[0]]
+    g = dict(nx=nx, ny=ny, nz=nz, xplanes=xp, yplanes=yp, zplanes=zp, cx=_f64(cx), cy=_f64(cy),
+             cell_univ=_i32(cell_univ).reshape(nz, ny, nx), bc=_i32(bc), n_univ=len(universes),
+             univ_nrings=nr, univ_radius=_f64(rad), univ_mat=_i32(mat),
+             mesh_n=_i32([len(mesh[0]) - 1, len(mesh[1]) - 1, len(mesh[2]) - 1]),
+             mesh_x=_f64(mesh[0]), mesh_y=_f64(mesh[1]), mesh_z=_f64(mesh[2]),
+             by_group=int(by_group), n_ebins=(len(e_edges) - 1 if e_edges is not None else 0),
+             e_edges=_f64(e_edges if e_edges is not None else [0.0]),
+             src_kind=int(src_kind), src_lo=_f64(src_lo), src_hi=_f64(src_hi),
+             src_dir_kind=0 if src_dir is None else 1, src_dir=_f64(src_dir if src_dir is not None else (0, 0, 1)),
+             src_energy_kind=ekind,
+             src_index=int(src_energy[1]) if ekind != 1 else 0,
+             src_energy=float(src_energy[1]) if ekind == 1 else 0.0,
+             tally_scale_log2=int(scale_log2))
+    return g
+
+
+def mg_materials(sig_t, sig_s, sig_f, nu, chi):
+    sig_t = _f64(sig_t)
+    n_mat, G = sig_t.shape
+    return dict(n_mat=n_mat, G=G, sig_t=sig_t, sig_s=_f64(sig_s).reshape(n_mat, G, G), sig_f=_f64(sig_f).reshape(n_mat, G),
+                nu=_f64(nu).reshape(n_mat, G), chi=_f64(chi).reshape(n_mat, G))
+
+
+def ce_materials(mats):
+    """mats: list of list of (nuclide index, atom density)."""
+    n_mat = len(mats)
+    nn = _i32([len(m) for m in mats])
+    nuc = np.zeros((n_mat, MAX_NUC), dtype=np.int32)
+    dens = np.zeros((n_mat, MAX_NUC))
+    for k, m in enumerate(mats):
+        for j, (n, d) in enumerate(m):
+            nuc[k, j] = n
+            dens[k, j] = d
+    return dict(n_mat=n_mat, G=0, mat_nnuc=nn, mat_nuc=_i32(nuc), mat_dens=_f64(dens))
+
+
+# --------------------------------------------------------------------------- pins / small problems
+def infinite_medium(sig_t, sig_s, sig_f=None, nu=None, chi=None, mode="fixed", n=100000,
+                    n_inactive=0, n_active=0, seed=1, by_group=0):
+    """Infinite homogeneous medium, point isotropic source at the origin, group 0."""
+    sig_t = np.atleast_1d(_f64(sig_t))
+    G = len(sig_t)
+    sig_s = _f64(sig_s).reshape(1, G, G)
+    sig_f = np.zeros((1, G)) if sig_f is None else _f64(sig_f).reshape(1, G)
+    nu = np.zeros((1, G)) if nu is None else _f64(nu).reshape(1, G)
+    chi = np.eye(1, G) if chi is None else _f64(chi).reshape(1, G)
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, by_group=by_group)
+    return Problem("infinite_medium", geo, mg_materials(sig_t.reshape(1, G), sig_s, sig_f, nu, chi), None,
+                   mode, n, n_inactive, n_active, seed)
+
+
+def cfg0(n=100000, seed=1):
+    """configs[0]: 1-group fixed source, St=1.0, Ss=0.7, analog capture."""
+    p = infinite_medium([1.0], [[0.7]], n=n, seed=seed)
+    p.name = "cfg0"
+    return p
+
+
+def slab(sig_t, L, n=100000, seed=1):
+    """Purely absorbing slab 0<x<L, mono-directional +x source at x=0, vacuum at x=L."""
+    geo = geometry([0.0, L], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6,
+                   src_dir=(1.0, 0.0, 0.0))
+    mats = mg_materials([[sig_t]], [[[0.0]]], [[0.0]], [[0.0]], [[1.0]])
+    return Problem("slab", geo, mats, None, "fixed", n, seed=seed)
+
+
+def _mg_material(rng, G, kind):
+    """One synthetic G-group material (recipe: DESIGN.md section 4, cfg1)."""
+    sig_t = rng.uniform(0.2, 2.0, G)
+    c = rng.uniform(0.50, 0.90, G) if kind == "fuel" else rng.uniform(0.90, 0.995, G)
+    P = np.zeros((G, G))
+    for g in range(G):
+        if g >= 4:
+            P[g, g - 1] = 0.05 * rng.uniform()
+        P[g, g] = 1.0
+        for j in range(1, G - g):
+            P[g, g + j] = 0.5 ** j * rng.uniform(0.5, 1.0)
+        P[g] /= P[g].sum()
+    sig_s = (c * sig_t)[:, None] * P
+    sig_a = sig_t - sig_s.sum(axis=1)
+    if kind == "fuel":
+        sig_f = rng.uniform(0.3, 0.7, G) * sig_a
+        nu = rng.uniform(2.3, 2.7, G)
+    elif kind == "chamber":
+        sig_f = 0.01 * sig_a
+        nu = np.full(G, 2.4)
+    else:
+        sig_f = np.zeros(G)
+        nu = np.zeros(G)
+    chi = np.zeros(G)
+    chi[:3] = (0.60, 0.30, 0.10)
+    return sig_t, sig_s, sig_f, nu, chi
+
+
+def _mg_set(kinds, G=7, seed=PROBLEM_SEED):
+    rng = np.random.default_rng(seed)
+    parts = [_mg_material(rng, G, k) for k in kinds]
+    return mg_materials(*[np.stack([p[i] for p in parts]) for i in range(5)])
+
+
+def cfg1(n=1000000, n_inactive=20, n_active=50, seed=1, identical_materials=False):
+    """configs[1]: 7-group k-eigenvalue 2-D pin cell, reflective."""
+    h = 0.63
+    geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((0.54,), (0, 1))], [1, 1, 1, 1, 0, 0],
+                   by_group=1, src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0))
+    mats = _mg_set(["fuel", "fuel"] if identical_materials else ["fuel", "mod"])
+    if identical_materials:
+        for k in ("sig_t", "sig_s", "sig_f", "nu", "chi"):
+            mats[k][1] = mats[k][0]
+    return Problem("cfg1", geo, mats, None, "k", n, n_inactive, n_active, seed)
+
+
+def cfg2(n=10000000, n_inactive=6, n_active=18, seed=1):
+    """configs[2]: 7-group k-eigenvalue, 3-D 2x2 assemblies in C5G7 *shape* (own pin rule)."""
+    pitch, npin = 1.26, 51
+    xp = np.arange(npin + 1) * pitch
+    zp = [0.0, 64.26, 85.68]
+    # materials: 0..3 fuels A-D, 4 guide tube, 5 fission chamber, 6 moderator
+    mats = _mg_set(["fuel", "fuel", "fuel", "fuel", "mod", "chamber", "mod"])
+    universes = [((0.54,), (m, 6)) for m in range(6)] + [((), (6,))]
+    MOD = 6
+    cu = np.full((2, npin, npin), MOD, dtype=np.int32)
+    for ay in range(2):
+        for ax in range(2):
+            for j in range(17):
+                for i in range(17):
+                    if (i, j) == (8, 8):
+                        u = 5
+                    elif i in (2, 5, 8, 11, 14) and j in (2, 5, 8, 11, 14):
+                        u = 4
+                    elif ax == ay:
+                        u = 0
+                    else:
+                        t = min(i, j, 16 - i, 16 - j)
+                        u = 1 if t == 0 else (2 if t <= 3 else 3)
+                    cu[0, ay * 17 + j, ax * 17 + i] = u
+    mz = np.linspace(0.0, 85.68, 10)
+    mz[-1] = 85.68
+    geo = geometry(xp, xp, zp, cu, universes, [1, 0, 1, 0, 1, 0], mesh=(xp, xp, mz), by_group=0,
+                   src_kind=1, src_lo=(0.0, 0.0, 0.0), src_hi=(42.84, 42.84, 64.26))
+    return Problem("cfg2", geo, mats, None, "k", n, n_inactive, n_active, seed)
+
+
+# --------------------------------------------------------------------------- continuous energy
+def ce_tables(n_grid=50000, n_res=200, sigf0=2.5, seed=PROBLEM_SEED):
+    """3 synthetic nuclides (A=1,16,238) on a log grid 1e-5 eV .. 2e7 eV."""
+    rng = np.random.default_rng(seed + 1)
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    inv_v = np.sqrt(0.0253 / E)
+    z = np.zeros(n_grid)
+    s = [np.full(n_grid, 20.0), np.full(n_grid, 3.8), np.full(n_grid, 9.0)]
+    c = [0.332 * inv_v, 1e-4 * inv_v, 2.7 * inv_v]
+    f = [z.copy(), z.copy(), sigf0 * inv_v + 0.3 * (E > 1e6)]
+    lo, hi = np.searchsorted(E, 1.0), np.searchsorted(E, 1e3)
+    idx = rng.integers(lo, hi, n_res)
+    gg = 0.023
+    for Er, xi in zip(E[idx], rng.uniform(size=n_res)):
+        gn = 2e-3 * (0.1 + 2 * xi * xi) * np.sqrt(Er)
+        gt = gn + gg
+        s0 = 2.608e6 / Er * (gn / gt)
+        x = 2.0 * (E - Er) / gt
+        lor = 1.0 / (1.0 + x * x)
+        s[2] = s[2] + s0 * (gn / gt) * lor
+        cap = s0 * (gg / gt) * np.sqrt(Er / E) * lor
+        c[2] = c[2] + cap
+        f[2] = f[2] + 0.05 * cap
+    return dict(n_grid=n_grid, n_nuc=3, energy=_f64(E), A=_f64([1.0, 16.0, 238.0]),
+                sig_s=_f64(np.stack(s)), sig_c=_f64(np.stack(c)), sig_f=_f64(np.stack(f)),
+                nu=_f64([0.0, 0.0, 2.43]), watt_a=_f64([1.0, 1.0, 0.988e6]), watt_b=_f64([1.0, 1.0, 2.249e-6]))
+
+
+def _ce_pin(n_ebins, n_grid, src_energy, sigf0):
+    h = 0.63
+    xs = ce_tables(n_grid=n_grid, sigf0=sigf0)
+    E = xs["energy"]
+    edges = E[np.round(np.arange(n_ebins + 1) * (n_grid - 1) / n_ebins).astype(int)]
+    geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((0.54,), (0, 1))], [1, 1, 1, 1, 0, 0],
+                   e_edges=edges, src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0), src_energy=src_energy)
+    mats = ce_materials([[(2, 0.022), (1, 0.044)], [(0, 0.0668), (1, 0.0334)]])
+    return geo, mats, xs
+
+
+CE_SIGF0 = 2.5   # thermal fission scale of the A=238 nuclide, tuned so k_inf < 1 (reading Q17)
+
+
+def cfg3(n=1000000, n_ebins=100, seed=1, n_grid=50000, sigf0=CE_SIGF0):
+    """configs[3]: continuous-energy infinite pin cell, fixed 14 MeV source, energy-mesh tally."""
+    geo, mats, xs = _ce_pin(n_ebins, n_grid, ("mono", 14e6), sigf0)
+    return Problem("cfg3", geo, mats, xs, "fixed", n, seed=seed)
+
+
+def cfg4(n=100000000, n_inactive=1, n_active=2, n_ebins=100, seed=1, n_grid=50000, sigf0=CE_SIGF0):
+    """configs[4]: the same pin cell in k-eigenvalue mode (generation-0 source: Watt of nuclide 2)."""
+    geo, mats, xs = _ce_pin(n_ebins, n_grid, ("watt", 2), sigf0)
+    return Problem("cfg4", geo, mats, xs, "k", n, n_inactive, n_active, seed)
+
+
+def ce_slowing_down(A=1.0, n=100000, n_grid=2000, seed=1, n_ebins=7):
+    """Pure scatterer of mass A (tiny 1/v capture), infinite medium, 1 MeV source: kinematics pin."""
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    xs = dict(n_grid=n_grid, n_nuc=1, energy=_f64(E), A=_f64([A]), sig_s=_f64(np.full((1, n_grid), 20.0)),
+              sig_c=_f64(np.zeros((1, n_grid))), sig_f=_f64(np.zeros((1, n_grid))),
+              nu=_f64([0.0]), watt_a=_f64([1.0]), watt_b=_f64([1.0]))
+    xs["sig_c"][0, :200] = 1e6        # absorb once thermal so histories end
+    edges = 10.0 ** np.arange(-1, n_ebins)            # decade bins 0.1 eV .. 1e6 eV
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, e_edges=edges,
+                   src_energy=("mono", 1e6))
+    return Problem("ce_slowing_down", geo, ce_materials([[(0, 0.05)]]), xs, "fixed", n, seed=seed)
+
+
+BY_NAME = {"cfg0": cfg0, "cfg1": cfg1, "cfg2": cfg2, "cfg3": cfg3, "cfg4": cfg4}
