@@ -1,0 +1,147 @@
+/* tdr.h — C ABI of the B200 event-based Monte Carlo transport library (libtdr.so).
+ *
+ * Method: event-based neutron transport with thread-data remapping (TDR), arxiv 2506.00263:
+ *   - stack-based remapping (section 3.1): per-event index stacks, warp-collective
+ *     push with one atomic per warp, one kernel launch per non-empty stack, make_work when drained;
+ *   - asynchronous remapping (section 3.2): one persistent kernel, per-warp stash of
+ *     work links in shared memory, spill/fetch through global link queues claimed by atomic swap;
+ *   - monolithic ("fused") and decomposed ("split") task schemes (section 4).
+ * The four calls named by BASELINE.json north_star are tdr_init_problem, tdr_run_fixed_source,
+ * tdr_run_k_eigenvalue and tdr_read_tallies; the rest make them usable.  The numbered readings
+ * (N,R,G,X,B,T,D) that fix the physics where the paper is silent are in DESIGN.md section 3.
+ *
+ * Conventions: every pointer inside tdr_geometry / tdr_materials / tdr_xs_tables is a HOST pointer;
+ * tdr_init_problem copies what it needs (the caller may free at once).  tdr_tallies holds HOST
+ * buffers allocated by the caller (sizes from tdr_tally_sizes; NULL = skip).  The only DEVICE
+ * pointer in the interface is the workspace given to tdr_bind_workspace, which stays owned by the
+ * caller (torch) and must outlive the runs.  All calls return 0 or a negative TDR_E* code and
+ * never throw; tdr_last_error() gives a thread-local message.  run_* return after the stream has
+ * drained.  There is no CPU fallback: without a CUDA device every run_* returns TDR_ECUDA.
+ */
+#ifndef TDR_H
+#define TDR_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TDR_MAX_RINGS 4
+#define TDR_MAX_NUC 4
+
+enum { TDR_OK = 0, TDR_EINVAL = -1, TDR_ENOMEM = -2, TDR_ECUDA = -3, TDR_ECAPACITY = -4, TDR_ELOST = -5,
+       TDR_EOVERFLOW = -6, TDR_ESTATE = -7 };
+
+/* Geometry (G1-G7): rectilinear lattice of nx*ny*nz cells; each cell holds a universe of
+ * concentric z-cylinders about (cx[ix], cy[iy]); tally mesh and source. */
+typedef struct tdr_geometry {
+  int32_t nx, ny, nz;
+  const double *xplanes, *yplanes, *zplanes; /* nx+1, ny+1, nz+1 ascending; outer ones may be +-inf */
+  const double *cx, *cy;                     /* nx, ny */
+  const int32_t *cell_univ;                  /* [nz][ny][nx] */
+  int32_t bc[6];                             /* faces -x,+x,-y,+y,-z,+z: 0 vacuum, 1 reflective */
+  int32_t n_univ;
+  const int32_t *univ_nrings;                /* n_univ, each <= TDR_MAX_RINGS */
+  const double *univ_radius;                 /* n_univ*TDR_MAX_RINGS ascending */
+  const int32_t *univ_mat;                   /* n_univ*(TDR_MAX_RINGS+1), ring 0 (innermost) .. nrings */
+  int32_t mesh_n[3];
+  const double *mesh_x, *mesh_y, *mesh_z;    /* mesh_n[a]+1 planes; must cover the lattice box */
+  int32_t by_group;                          /* multigroup: tally energy axis = group */
+  int32_t n_ebins;                           /* continuous energy: number of energy bins */
+  const double *e_edges;                     /* n_ebins+1 */
+  int32_t src_kind;                          /* 0 point at src_lo, 1 uniform box [src_lo, src_hi] */
+  double src_lo[3], src_hi[3];
+  int32_t src_dir_kind;                      /* 0 isotropic, 1 fixed src_dir */
+  double src_dir[3];
+  int32_t src_energy_kind;                   /* 0 group src_index, 1 mono src_energy, 2 Watt of nuclide src_index */
+  int32_t src_index;
+  double src_energy;
+  int32_t tally_scale_log2;                  /* S: tallies are llrint(v * 2^S) summed in int64 */
+} tdr_geometry;
+
+typedef struct tdr_materials {
+  int32_t n_mat;
+  int32_t G;                                 /* groups; 0 = continuous energy */
+  const double *sig_t, *sig_s, *sig_f, *nu, *chi; /* MG: [m][g], [m][g from][g to], [m][g] */
+  const int32_t *mat_nnuc;                   /* CE: n_mat */
+  const int32_t *mat_nuc;                    /* CE: n_mat*TDR_MAX_NUC nuclide indices */
+  const double *mat_dens;                    /* CE: n_mat*TDR_MAX_NUC atom densities (1/b-cm) */
+} tdr_materials;
+
+typedef struct tdr_xs_tables {               /* CE only; NULL for multigroup */
+  int32_t n_grid, n_nuc;
+  const double *energy;                      /* n_grid strictly increasing (union grid) */
+  const double *A;                           /* n_nuc */
+  const double *sig_s, *sig_c, *sig_f;       /* [nuc][n_grid] barns */
+  const double *nu, *watt_a, *watt_b;        /* n_nuc */
+} tdr_xs_tables;
+
+typedef struct tdr_site {                    /* fission-bank / source-bank record, 48 bytes */
+  double x, y, z;
+  uint64_t id;
+  int16_t ix, iy, iz, mx, my, mz;
+  uint8_t ring, src, depth, pad;
+} tdr_site;
+
+typedef struct tdr_sizes {
+  uint64_t n_bins;                           /* flux / coll length */
+  uint64_t n_gen;                            /* generations run (0 after a fixed-source run) */
+  uint64_t n_hist;                           /* per-history records kept */
+  uint64_t n_bank;                           /* sites in the last generation's fission bank */
+} tdr_sizes;
+
+enum { TDR_T_NSEG = 0, TDR_T_NCOLL, TDR_T_NCROSS, TDR_T_NABS, TDR_T_NFIS, TDR_T_NLEAK, TDR_T_NBORN,
+       TDR_T_NDROPPED, TDR_T_NDIRFAIL, TDR_T_DIGEST, TDR_T_NSITES, TDR_T_COUNT = 12 };
+
+typedef struct tdr_tallies {                 /* HOST buffers, caller-allocated; NULL = skip */
+  int64_t *flux, *coll;                      /* n_bins, bin = ((mz*ny_m+my)*nx_m+mx)*n_e + e */
+  int64_t leak[6];
+  uint64_t totals[TDR_T_COUNT];
+  double k_mean, k_std;
+  uint64_t *gen_n, *gen_m;                   /* n_gen: starters, bank sites */
+  int64_t *gen_p, *gen_pc;                   /* n_gen: track-length / collision production, fixed point */
+  double *gen_k;                             /* n_gen */
+  uint64_t *hist_id; uint32_t *hist_nseg, *hist_ncoll; /* n_hist, any order */
+  tdr_site *bank;                            /* n_bank, any order */
+} tdr_tallies;
+
+typedef struct tdr_diag {
+  uint64_t kernel_launches;                  /* kernels launched by the last run_* */
+  uint64_t iterations;                       /* stack scheme: remap iterations; async: persistent launches */
+  uint64_t events[8];                        /* kernel-level events: source, step|lookup, move, tally, collide, surface, popctrl, - */
+  uint64_t spills, fetches, make_work_calls; /* async scheme */
+  double gpu_ms;                             /* CUDA-event time of the last run_* body */
+  double step_ms;                            /* CUDA-event time summed over the dominant kernel's launches */
+  uint64_t step_launches;
+} tdr_diag;
+
+typedef struct tdr_problem tdr_problem;
+
+/* Copy the problem to the device, derive tables (MG cdfs, CE hash).  TDR_EINVAL on bad input. */
+int tdr_init_problem(const tdr_geometry *, const tdr_materials *, const tdr_xs_tables *, tdr_problem **out);
+/* keys: "scheme" = stack|async; "decomposition" = fused|split; "window" = particles in flight;
+ * "stash_links" (async, links per warp); "blocks_per_sm"; "keep_history" = 0|1. */
+int tdr_set_option(tdr_problem *, const char *key, const char *value);
+int tdr_workspace_bytes(const tdr_problem *, uint64_t n_particles, uint64_t *bytes);
+/* device_ptr: DEVICE memory of at least `bytes` (256-byte aligned); cuda_stream: cudaStream_t. */
+int tdr_bind_workspace(tdr_problem *, void *device_ptr, uint64_t bytes, void *cuda_stream);
+/* D1: ids 0..n-1, generation 0, secondaries followed to extinction. */
+int tdr_run_fixed_source(tdr_problem *, uint64_t n_particles, uint64_t seed);
+/* D2: power iteration with population control; tallies over active generations. */
+int tdr_run_k_eigenvalue(tdr_problem *, uint64_t n_particles, uint32_t n_inactive, uint32_t n_active, uint64_t seed);
+int tdr_tally_sizes(const tdr_problem *, tdr_sizes *out);
+/* Copies device tallies into the caller's HOST buffers.  TDR_ESTATE before any run. */
+int tdr_read_tallies(const tdr_problem *, tdr_tallies *out);
+int tdr_read_diagnostics(const tdr_problem *, tdr_diag *out);
+void tdr_free_problem(tdr_problem *);
+const char *tdr_last_error(void);
+
+/* Unit-level device entry points (used by the parity tests of the primitives): all pointers DEVICE.
+ * out[i] = det_log(x[i]); out[i] = draw(seed, id[i], gen, seg, purpose, j). */
+int tdr_dev_det_log(const double *x, double *out, uint64_t n, void *cuda_stream);
+int tdr_dev_draw(uint64_t seed, const uint64_t *id, uint32_t gen, uint32_t seg, uint32_t purpose, uint32_t j,
+                 double *out, uint64_t n, void *cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,467 @@
+// tdr_api.cu — C ABI (include/tdr.h) and host drivers (D1 fixed source, D2 k-eigenvalue) of libtdr.so.
+// Build: nvcc -gencode arch=compute_100a,code=sm_100a -O3 -fmad=false -lineinfo -shared -Xcompiler -fPIC
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <string>
+#include <vector>
+#include "tdr_stack.cuh"
+#include "tdr_split.cuh"
+#include "tdr_async.cuh"
+
+static thread_local char g_err[512] = "";
+static int fail(int code, const char *fmt, ...) {
+  va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof g_err, fmt, ap); va_end(ap);
+  return code;
+}
+#define CK(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) return fail(TDR_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); } while (0)
+
+struct tdr_problem {
+  DevProb dp;
+  std::vector<void *> dev_allocs;          // problem tables (cudaMalloc'd at init)
+  bool ce = false;
+  int S = 24;
+  // options
+  int scheme = 0;                          // 0 stack, 1 async
+  int split = 0;                           // 0 fused, 1 split
+  u64 window = 1ull << 20;
+  int stash_links = 8;
+  int blocks_per_sm = 0;                   // 0 = occupancy query
+  int keep_history = -1;                   // -1 auto (n <= 2e6)
+  int time_kernels = 0;
+  // workspace
+  char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
+  // carved pointers (valid during/after a run)
+  Soa soa; u32 *stacks[EV_COUNT]; u64 *ctr; DevOut out; tdr_site *bank, *srcbank, *sec;
+  u64 bank_cap = 0, src_cap = 0, sec_cap = 0, hist_cap = 0, W = 0;
+  u64 *hist_id; u32 *hist_nseg, *hist_ncoll;
+  AsyncMem am;
+  // results on host
+  bool ran = false;
+  std::vector<u64> gen_n, gen_m; std::vector<i64> gen_p, gen_pc; std::vector<double> gen_k;
+  double k_mean = 0, k_std = 0; u64 n_hist = 0, n_bank = 0;
+  tdr_diag diag;
+  int num_sms = 148;
+  u64 *h_ctr = nullptr;                    // pinned readback
+  std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
+};
+
+const char *tdr_last_error(void) { return g_err; }
+
+template <class T>
+static int upload(tdr_problem *p, const T *src, size_t n, const T **dst) {
+  void *d = nullptr;
+  size_t bytes = (n ? n : 1) * sizeof(T);
+  CK(cudaMalloc(&d, bytes));
+  p->dev_allocs.push_back(d);
+  if (n) CK(cudaMemcpy(d, src, n * sizeof(T), cudaMemcpyHostToDevice));
+  *dst = (const T *)d;
+  return 0;
+}
+
+void tdr_free_problem(tdr_problem *p) {
+  if (!p) return;
+  for (void *d : p->dev_allocs) cudaFree(d);
+  for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
+  if (p->h_ctr) cudaFreeHost(p->h_ctr);
+  delete p;
+}
+
+int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs_tables *x, tdr_problem **out) {
+  if (!g || !m || !out) return fail(TDR_EINVAL, "null argument");
+  if (g->nx < 1 || g->ny < 1 || g->nz < 1 || g->n_univ < 1 || m->n_mat < 1) return fail(TDR_EINVAL, "empty geometry or materials");
+  if (g->nx > 32767 || g->ny > 32767 || g->nz > 32767) return fail(TDR_EINVAL, "lattice too large for 16-bit indices");
+  if (m->n_mat > 255 || m->G > 255 || m->G < 0) return fail(TDR_EINVAL, "too many materials or groups");
+  if (m->G == 0 && !x) return fail(TDR_EINVAL, "continuous energy needs xs_tables");
+  if (g->tally_scale_log2 < 0 || g->tally_scale_log2 > 40) return fail(TDR_EINVAL, "tally_scale_log2 out of range");
+  const double *mp[3] = { g->mesh_x, g->mesh_y, g->mesh_z };
+  const double *lp[3] = { g->xplanes, g->yplanes, g->zplanes };
+  const int ln[3] = { g->nx, g->ny, g->nz };
+  for (int a = 0; a < 3; a++) {
+    if (g->mesh_n[a] < 1 || g->mesh_n[a] > 32767) return fail(TDR_EINVAL, "bad mesh size");
+    if (!(mp[a][0] <= lp[a][0]) || !(mp[a][g->mesh_n[a]] >= lp[a][ln[a]])) return fail(TDR_EINVAL, "tally mesh must cover the lattice box");
+  }
+  for (int u = 0; u < g->n_univ; u++)
+    if (g->univ_nrings[u] < 0 || g->univ_nrings[u] > TDR_MAX_RINGS) return fail(TDR_EINVAL, "bad ring count");
+  int dev_count = 0;
+  if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) return fail(TDR_ECUDA, "no CUDA device: this library has no CPU fallback");
+  tdr_problem *p = new tdr_problem();
+  memset(&p->dp, 0, sizeof p->dp); memset(&p->diag, 0, sizeof p->diag); memset(&p->soa, 0, sizeof p->soa);
+  DevProb &D = p->dp;
+  int rc = 0;
+#define UP(src, n, dst) if (!rc) rc = upload(p, src, (size_t)(n), &dst)
+  D.nx = g->nx; D.ny = g->ny; D.nz = g->nz; D.n_univ = g->n_univ; D.G = m->G; D.n_mat = m->n_mat; D.by_group = g->by_group;
+  memcpy(D.bc, g->bc, sizeof D.bc); memcpy(D.mesh_n, g->mesh_n, sizeof D.mesh_n);
+  UP(g->xplanes, g->nx + 1, D.xp); UP(g->yplanes, g->ny + 1, D.yp); UP(g->zplanes, g->nz + 1, D.zp);
+  UP(g->cx, g->nx, D.cx); UP(g->cy, g->ny, D.cy);
+  UP(g->cell_univ, (size_t)g->nx * g->ny * g->nz, D.cell_univ);
+  UP(g->univ_nrings, g->n_univ, D.univ_nr); UP(g->univ_radius, g->n_univ * TDR_MAX_RINGS, D.univ_rad);
+  UP(g->univ_mat, g->n_univ * (TDR_MAX_RINGS + 1), D.univ_mat);
+  for (int a = 0; a < 3; a++) UP(mp[a], g->mesh_n[a] + 1, D.mesh[a]);
+  D.src_kind = g->src_kind; D.src_dir_kind = g->src_dir_kind; D.src_energy_kind = g->src_energy_kind; D.src_index = g->src_index;
+  memcpy(D.src_lo, g->src_lo, 24); memcpy(D.src_hi, g->src_hi, 24); memcpy(D.src_dir, g->src_dir, 24);
+  D.src_energy = g->src_energy; D.scale = ldexp(1.0, g->tally_scale_log2); p->S = g->tally_scale_log2;
+  p->ce = (m->G == 0);
+  if (!p->ce) {
+    D.n_e = g->by_group ? m->G : 1;
+    // X1: derived rows [sig_t, sig_s_tot, sig_c, nu*sig_f, nu, cdf...] + chi cdf
+    int G = m->G, M = m->n_mat, row = MGROW(G);
+    std::vector<double> t((size_t)M * G * row + (size_t)M * G);
+    for (int k = 0; k < M; k++) {
+      double cc = 0.0;
+      for (int a = 0; a < G; a++) {
+        double *r = &t[(size_t)(k * G + a) * row];
+        double acc = 0.0;
+        for (int b = 0; b < G; b++) { acc = acc + m->sig_s[(k * G + a) * G + b]; r[5 + b] = acc; }
+        double st = m->sig_t[k * G + a], sf = m->sig_f[k * G + a], nu = m->nu[k * G + a];
+        double sa = st - acc;
+        r[0] = st; r[1] = acc; r[2] = sa - sf; r[3] = nu * sf; r[4] = nu;
+        cc = cc + m->chi[k * G + a]; t[(size_t)M * G * row + k * G + a] = cc;
+      }
+    }
+    D.mg_doubles = (int)t.size();
+    UP(t.data(), t.size(), D.mg);
+  } else {
+    if (g->n_ebins < 1 || x->n_grid < 2 || x->n_nuc < 1 || x->n_nuc > 255) { tdr_free_problem(p); return fail(TDR_EINVAL, "bad CE tables"); }
+    D.n_e = g->n_ebins; UP(g->e_edges, g->n_ebins + 1, D.e_edges);
+    D.n_grid = x->n_grid; D.n_nuc = x->n_nuc;
+    UP(m->mat_nnuc, m->n_mat, D.mat_nnuc); UP(m->mat_nuc, m->n_mat * TDR_MAX_NUC, D.mat_nuc); UP(m->mat_dens, m->n_mat * TDR_MAX_NUC, D.mat_dens);
+    UP(x->energy, x->n_grid, D.grid); UP(x->A, x->n_nuc, D.A); UP(x->nu, x->n_nuc, D.nuc_nu); UP(x->watt_a, x->n_nuc, D.wa); UP(x->watt_b, x->n_nuc, D.wb);
+    std::vector<double4> rec((size_t)x->n_nuc * x->n_grid);
+    for (size_t i = 0; i < rec.size(); i++) rec[i] = make_double4(x->sig_s[i], x->sig_c[i], x->sig_f[i], 0.0);
+    UP(rec.data(), rec.size(), D.xs);
+    D.grid_lo = x->energy[0]; D.grid_hi = x->energy[x->n_grid - 1];
+    if (!(D.grid_lo > 0.0)) { tdr_free_problem(p); return fail(TDR_EINVAL, "energy grid must be positive"); }
+    // X3: bucket = top bits (exponent + 7 mantissa bits) of E; hash[b] = largest i with grid[i] <= lower edge of b
+    u64 blo, bhi; memcpy(&blo, &D.grid_lo, 8); memcpy(&bhi, &D.grid_hi, 8);
+    D.hash_bmin = (u32)(blo >> 45); D.hash_n = (u32)(bhi >> 45) - D.hash_bmin + 1;
+    std::vector<u32> h(D.hash_n + 1);
+    int i = 0;
+    for (u32 b = 0; b <= D.hash_n; b++) {
+      u64 eb = ((u64)(D.hash_bmin + b)) << 45; double edge; memcpy(&edge, &eb, 8);
+      while (i + 1 < x->n_grid && x->energy[i + 1] <= edge) i++;
+      h[b] = (u32)i;
+    }
+    UP(h.data(), h.size(), D.hash);
+  }
+#undef UP
+  if (rc) { tdr_free_problem(p); return rc; }
+  D.n_bins = (u64)D.mesh_n[0] * D.mesh_n[1] * D.mesh_n[2] * D.n_e;
+  cudaDeviceProp prop; int dev = 0; cudaGetDevice(&dev);
+  if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) p->num_sms = prop.multiProcessorCount;
+  if (cudaMallocHost((void **)&p->h_ctr, 64 * sizeof(u64)) != cudaSuccess) { tdr_free_problem(p); return fail(TDR_ECUDA, "cudaMallocHost failed"); }
+  *out = p;
+  return TDR_OK;
+}
+
+int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
+  if (!p || !key || !value) return fail(TDR_EINVAL, "null argument");
+  std::string k(key), v(value);
+  if (k == "scheme") { if (v == "stack") p->scheme = 0; else if (v == "async") p->scheme = 1; else return fail(TDR_EINVAL, "scheme must be stack|async"); }
+  else if (k == "decomposition") { if (v == "fused") p->split = 0; else if (v == "split") p->split = 1; else return fail(TDR_EINVAL, "decomposition must be fused|split"); }
+  else if (k == "window") { long long w = atoll(value); if (w < 32) return fail(TDR_EINVAL, "window too small"); p->window = (u64)w; }
+  else if (k == "stash_links") { int n = atoi(value); if (n < 4 || n > 64) return fail(TDR_EINVAL, "stash_links in [4,64]"); p->stash_links = n; }
+  else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
+  else if (k == "keep_history") p->keep_history = atoi(value);
+  else if (k == "time_kernels") p->time_kernels = atoi(value);
+  else return fail(TDR_EINVAL, "unknown option %s", key);
+  return TDR_OK;
+}
+
+// ---------------------------------------------------------------------------------- workspace layout
+struct Carver {
+  char *base; u64 off = 0;
+  template <class T> T *take(u64 n) { off = (off + 255) & ~255ull; T *r = base ? (T *)(base + off) : nullptr; off += n * sizeof(T); return r; }
+};
+
+static u64 window_for(const tdr_problem *p, u64 n) {
+  u64 cap = n + n / 4 + 4096;                 // k-mode population floats around n
+  u64 w = p->window < cap ? p->window : cap;
+  return (w + 31) & ~31ull;
+}
+
+static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
+  Carver c; c.base = base;
+  u64 W = window_for(p, n);
+  Soa s; memset(&s, 0, sizeof s);
+  s.x = c.take<double>(W); s.y = c.take<double>(W); s.z = c.take<double>(W);
+  s.u = c.take<double>(W); s.v = c.take<double>(W); s.w = c.take<double>(W);
+  s.E = c.take<double>(p->ce ? W : 1);
+  s.id = c.take<u64>(W); s.loc0 = c.take<u64>(W); s.loc1 = c.take<u64>(W);
+  s.seg = c.take<u32>(W); s.ncoll = c.take<u32>(W);
+  s.s_sigt = c.take<double>(W); s.s_nsf = c.take<double>(W); s.s_d = c.take<double>(W); s.s_f = c.take<double>(W);
+  s.s_flags = c.take<u32>(W); s.s_gi = c.take<u32>(W);
+  u32 *st[EV_COUNT];
+  for (int e = 0; e < EV_COUNT; e++) st[e] = c.take<u32>(W);
+  u64 *ctr = c.take<u64>(C_COUNT);
+  DevOut o;
+  o.flux = c.take<u64>(p->dp.n_bins); o.coll = c.take<u64>(p->dp.n_bins); o.leak = c.take<u64>(6);
+  o.totals = c.take<u64>(TDR_T_COUNT); o.PPc = c.take<u64>(2); o.err = c.take<int>(1);
+  u64 bank_cap = 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + 4096;
+  tdr_site *bank = c.take<tdr_site>(bank_cap), *src = c.take<tdr_site>(src_cap), *sec = c.take<tdr_site>(sec_cap);
+  u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
+  u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
+  AsyncMem am; async_layout(c, W, p->num_sms, am);
+  if (assign) {
+    p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
+    p->bank = bank; p->srcbank = src; p->sec = sec; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
+    p->hist_cap = hist_cap; p->hist_id = hid; p->hist_nseg = hs; p->hist_ncoll = hc; p->am = am;
+  }
+  return (c.off + 255) & ~255ull;
+}
+
+int tdr_workspace_bytes(const tdr_problem *p, uint64_t n, uint64_t *bytes) {
+  if (!p || !bytes || n == 0) return fail(TDR_EINVAL, "bad argument");
+  *bytes = layout(const_cast<tdr_problem *>(p), n, nullptr, false);
+  return TDR_OK;
+}
+
+int tdr_bind_workspace(tdr_problem *p, void *ptr, uint64_t bytes, void *stream) {
+  if (!p || !ptr || ((uintptr_t)ptr & 255)) return fail(TDR_EINVAL, "workspace must be a 256-byte aligned device pointer");
+  cudaPointerAttributes at;
+  if (cudaPointerGetAttributes(&at, ptr) != cudaSuccess || at.type != cudaMemoryTypeDevice) { cudaGetLastError(); return fail(TDR_EINVAL, "workspace is not device memory"); }
+  p->ws = (char *)ptr; p->ws_bytes = bytes; p->stream = (cudaStream_t)stream;
+  return TDR_OK;
+}
+
+// ---------------------------------------------------------------------------------- launch helpers
+template <class K>
+static int grid_for(tdr_problem *p, K kernel, size_t smem, int threads = 256) {
+  int bps = p->blocks_per_sm;
+  if (bps <= 0) { if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, threads, smem) != cudaSuccess || bps < 1) bps = 1; }
+  return p->num_sms * bps;
+}
+
+struct KTimer {                                   // optional CUDA-event bracket around the dominant kernel's launches
+  tdr_problem *p; bool on;
+  KTimer(tdr_problem *p_, bool dominant) : p(p_), on(p_->time_kernels && dominant) {
+    if (!on) return;
+    while (p->ev_pool.size() < p->ev_used + 2) { cudaEvent_t e; cudaEventCreate(&e); p->ev_pool.push_back(e); }
+    cudaEventRecord(p->ev_pool[p->ev_used], p->stream);
+  }
+  ~KTimer() { if (on) { cudaEventRecord(p->ev_pool[p->ev_used + 1], p->stream); p->ev_used += 2; p->diag.step_launches++; } }
+};
+
+static void collect_kernel_times(tdr_problem *p) {
+  double ms = 0;
+  for (size_t i = 0; i + 1 < p->ev_used; i += 2) { float t = 0; cudaEventElapsedTime(&t, p->ev_pool[i], p->ev_pool[i + 1]); ms += t; }
+  p->diag.step_ms = ms; p->ev_used = 0;
+}
+
+static int check_dev_err(tdr_problem *p, int code) {
+  if (code == 0) return 0;
+  const char *w = code == TDR_ECAPACITY ? "bank/stack/arena capacity exceeded" : code == TDR_ELOST ? "lost particle (no finite distance or segment overflow)" : "device error";
+  return fail(code, "%s", w);
+}
+
+#define LAUNCH_CHECK() CK(cudaGetLastError())
+
+// ---------------------------------------------------------------------------------- stack scheme, one generation
+template <bool CE>
+static int run_stack(tdr_problem *p, DevRun R) {
+  cudaStream_t st = p->stream;
+  const size_t smem = (size_t)p->dp.mg_doubles * sizeof(double);
+  u64 *ctr = p->ctr; u64 *h = p->h_ctr, *hup = p->h_ctr + 32;
+  const int g_src = grid_for(p, k_source<CE>, smem);
+  const u64 W = p->W;
+  u64 h_src_next = 0, h_sec_tail = 0, h_sec_head = 0;
+  auto source = [&](u32 *stack, u64 *count, u64 n_sec, u64 n) -> int {
+    k_source<CE><<<g_src, 256, smem, st>>>(p->dp, p->out, R, p->soa, stack, count, h_sec_head, n_sec, h_src_next, n);
+    LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.events[0] += n;
+    h_sec_head += n_sec; h_src_next += n - n_sec;
+    hup[0] = h_src_next; hup[1] = h_sec_head;
+    CK(cudaMemcpyAsync(ctr + C_SRC_NEXT, hup, 8, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, hup + 1, 8, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));                 // hup is reused
+    return 0;
+  };
+  int rc;
+  u64 n0 = R.src_total < W ? R.src_total : W;
+  const int first = p->split ? EV_LOOKUP : 0;
+  if ((rc = source(p->stacks[first], ctr + C_STACK0 + first, 0, n0))) return rc;
+  int cur = 0;
+  const int g_step = grid_for(p, k_step<CE>, smem);
+  SplitGrids sg; if (p->split) split_grids<CE>(p, smem, sg);
+  for (;;) {
+    R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
+    u64 alive;
+    if (!p->split) {
+      CK(cudaMemsetAsync(ctr + C_STACK0 + (1 - cur), 0, 8, st));
+      {
+        KTimer t(p, true);
+        k_step<CE><<<g_step, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[cur], ctr + C_STACK0 + cur, p->stacks[1 - cur], ctr + C_STACK0 + 1 - cur);
+      }
+      LAUNCH_CHECK(); p->diag.kernel_launches++;
+      cur = 1 - cur;
+    } else {
+      if ((rc = split_iteration<CE>(p, R, smem, sg))) return rc;
+    }
+    p->diag.iterations++;
+    CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
+    alive = p->split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + cur];
+    p->diag.events[1] += alive;
+    h_sec_tail = h[C_SEC_TAIL];
+    h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
+    u64 head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;
+    if (head != h[C_SEC_HEAD]) { hup[1] = head; CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, hup + 1, 8, cudaMemcpyHostToDevice, st)); CK(cudaStreamSynchronize(st)); }
+    h_sec_head = head;
+    if (alive == 0) {
+      u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
+      if (pend + rem == 0) break;
+      u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;
+      int slot = p->split ? EV_LOOKUP : cur;
+      if ((rc = source(p->stacks[slot], ctr + C_STACK0 + slot, n_sec, n))) return rc;
+    }
+  }
+  return 0;
+}
+
+// one generation (or the whole fixed-source run) under the selected scheme
+static int run_generation(tdr_problem *p, DevRun &R) {
+  cudaStream_t st = p->stream;
+  CK(cudaMemsetAsync(p->ctr, 0, C_COUNT * 8, st));
+  CK(cudaMemsetAsync(p->out.PPc, 0, 16, st));
+  R.src_next = p->ctr + C_SRC_NEXT; R.sec_tail = p->ctr + C_SEC_TAIL; R.sec_head = p->ctr + C_SEC_HEAD;
+  R.bank_count = p->ctr + C_BANK; R.hist_count = p->ctr + C_HIST;
+  R.sec = p->sec; R.sec_cap = p->sec_cap; R.sec_limit = 0; R.sec_head0 = 0;
+  R.bank = p->bank; R.bank_cap = p->bank_cap;
+  R.hist_id = p->hist_id; R.hist_nseg = p->hist_nseg; R.hist_ncoll = p->hist_ncoll;
+  if (p->scheme == 0) return p->ce ? run_stack<true>(p, R) : run_stack<false>(p, R);
+  return p->ce ? run_async<true>(p, R) : run_async<false>(p, R);
+}
+
+static int begin_run(tdr_problem *p, u64 n) {
+  if (!p || n == 0) return fail(TDR_EINVAL, "bad argument");
+  if (!p->ws) return fail(TDR_ESTATE, "no workspace bound (tdr_bind_workspace)");
+  u64 need = layout(p, n, nullptr, false);
+  if (need > p->ws_bytes) return fail(TDR_ENOMEM, "workspace too small: need %llu bytes, have %llu", need, (u64)p->ws_bytes);
+  layout(p, n, p->ws, true);
+  p->out.err = (int *)(p->ctr + (C_COUNT - 1));
+  cudaStream_t st = p->stream;
+  CK(cudaMemsetAsync(p->out.flux, 0, p->dp.n_bins * 8, st)); CK(cudaMemsetAsync(p->out.coll, 0, p->dp.n_bins * 8, st));
+  CK(cudaMemsetAsync(p->out.leak, 0, 48, st)); CK(cudaMemsetAsync(p->out.totals, 0, TDR_T_COUNT * 8, st));
+  p->ran = false; p->gen_n.clear(); p->gen_m.clear(); p->gen_p.clear(); p->gen_pc.clear(); p->gen_k.clear();
+  p->k_mean = p->k_std = 0; p->n_hist = p->n_bank = 0;
+  memset(&p->diag, 0, sizeof p->diag); p->ev_used = 0;
+  return 0;
+}
+
+struct RunClock {
+  cudaEvent_t a, b; cudaStream_t st;
+  RunClock(cudaStream_t s) : st(s) { cudaEventCreate(&a); cudaEventCreate(&b); cudaEventRecord(a, st); }
+  double stop() { cudaEventRecord(b, st); cudaEventSynchronize(b); float ms = 0; cudaEventElapsedTime(&ms, a, b); return ms; }
+  ~RunClock() { cudaEventDestroy(a); cudaEventDestroy(b); }
+};
+
+int tdr_run_fixed_source(tdr_problem *p, uint64_t n, uint64_t seed) {
+  int rc = begin_run(p, n); if (rc) return rc;
+  RunClock clk(p->stream);
+  DevRun R; memset(&R, 0, sizeof R);
+  R.seed = seed; R.gen = 0; R.kmode = 0; R.active = 1; R.k_prev = 1.0; R.src_sites = 0; R.sites = nullptr; R.src_total = n;
+  bool keep = p->keep_history < 0 ? n <= 2000000 : p->keep_history != 0;
+  R.hist_cap = keep ? p->hist_cap : 0;
+  if ((rc = run_generation(p, R))) return rc;
+  CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, p->stream));
+  p->diag.gpu_ms = clk.stop();
+  collect_kernel_times(p);
+  if (keep && p->h_ctr[C_HIST] > p->hist_cap) return fail(TDR_ECAPACITY, "history record buffer overflow");
+  p->n_hist = keep ? p->h_ctr[C_HIST] : 0;
+  p->ran = true;
+  return TDR_OK;
+}
+
+int tdr_run_k_eigenvalue(tdr_problem *p, uint64_t n, uint32_t n_inactive, uint32_t n_active, uint64_t seed) {
+  if ((u64)n_inactive + n_active == 0 || (u64)n_inactive + n_active > 65535) return fail(TDR_EINVAL, "bad generation counts");
+  int rc = begin_run(p, n); if (rc) return rc;
+  RunClock clk(p->stream);
+  cudaStream_t st = p->stream;
+  const u32 n_gen = n_inactive + n_active;
+  u64 n_src = n; double k_prev = 1.0;
+  bool keep = p->keep_history < 0 ? n <= 2000000 : p->keep_history != 0;
+  for (u32 g = 0; g < n_gen; g++) {
+    DevRun R; memset(&R, 0, sizeof R);
+    R.seed = seed; R.gen = g; R.kmode = 1; R.active = g >= n_inactive; R.k_prev = k_prev;
+    R.src_sites = g > 0; R.sites = p->srcbank; R.src_total = n_src;
+    bool last = g + 1 == n_gen;
+    R.hist_cap = (keep && last) ? p->hist_cap : 0;
+    if ((rc = run_generation(p, R))) return rc;
+    CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(p->h_ctr + 16, p->out.PPc, 16, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    u64 M = p->h_ctr[C_BANK]; i64 P = (i64)p->h_ctr[16], Pc = (i64)p->h_ctr[17];
+    if (M > p->bank_cap) return fail(TDR_ECAPACITY, "fission bank overflow");
+    double k = ((double)P * (1.0 / p->dp.scale)) / (double)n_src;                    // D2
+    p->gen_n.push_back(n_src); p->gen_m.push_back(M); p->gen_p.push_back(P); p->gen_pc.push_back(Pc); p->gen_k.push_back(k);
+    if (M == 0) return fail(TDR_ESTATE, "fission bank empty in generation %u", g);
+    if (last) { p->n_bank = M; p->n_hist = R.hist_cap ? p->h_ctr[C_HIST] : 0; break; }
+    double pr = (double)n / (double)M;
+    CK(cudaMemsetAsync(p->ctr + C_NEXT_BANK, 0, 8, st));
+    k_popctrl<<<p->num_sms * 4, 256, 0, st>>>(p->bank, M, p->srcbank, p->src_cap, p->ctr + C_NEXT_BANK, seed, g + 1, pr, p->out.err);
+    LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.events[6] += M;
+    CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if ((rc = check_dev_err(p, (int)p->h_ctr[C_COUNT - 1]))) return rc;
+    n_src = p->h_ctr[C_NEXT_BANK]; k_prev = k;
+    if (n_src == 0) return fail(TDR_ESTATE, "population died out");
+  }
+  p->diag.gpu_ms = clk.stop();
+  collect_kernel_times(p);
+  double sum = 0.0;
+  for (u32 g = n_inactive; g < n_gen; g++) sum = sum + p->gen_k[g];
+  p->k_mean = n_active ? sum / (double)n_active : 0.0;
+  double var = 0.0;
+  for (u32 g = n_inactive; g < n_gen; g++) { double dk = p->gen_k[g] - p->k_mean; var = var + dk * dk; }
+  p->k_std = n_active > 1 ? sqrt((var / (double)(n_active - 1)) / (double)n_active) : 0.0;
+  p->ran = true;
+  return TDR_OK;
+}
+
+int tdr_tally_sizes(const tdr_problem *p, tdr_sizes *o) {
+  if (!p || !o) return fail(TDR_EINVAL, "null argument");
+  o->n_bins = p->dp.n_bins; o->n_gen = p->gen_n.size(); o->n_hist = p->n_hist; o->n_bank = p->n_bank;
+  return TDR_OK;
+}
+
+int tdr_read_tallies(const tdr_problem *p, tdr_tallies *t) {
+  if (!p || !t) return fail(TDR_EINVAL, "null argument");
+  if (!p->ran) return fail(TDR_ESTATE, "no completed run");
+  cudaStream_t st = p->stream;
+  if (t->flux) CK(cudaMemcpyAsync(t->flux, p->out.flux, p->dp.n_bins * 8, cudaMemcpyDeviceToHost, st));
+  if (t->coll) CK(cudaMemcpyAsync(t->coll, p->out.coll, p->dp.n_bins * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(t->leak, p->out.leak, 48, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(t->totals, p->out.totals, TDR_T_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  if (t->hist_id && p->n_hist) CK(cudaMemcpyAsync(t->hist_id, p->hist_id, p->n_hist * 8, cudaMemcpyDeviceToHost, st));
+  if (t->hist_nseg && p->n_hist) CK(cudaMemcpyAsync(t->hist_nseg, p->hist_nseg, p->n_hist * 4, cudaMemcpyDeviceToHost, st));
+  if (t->hist_ncoll && p->n_hist) CK(cudaMemcpyAsync(t->hist_ncoll, p->hist_ncoll, p->n_hist * 4, cudaMemcpyDeviceToHost, st));
+  if (t->bank && p->n_bank) CK(cudaMemcpyAsync(t->bank, p->bank, p->n_bank * sizeof(tdr_site), cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  t->k_mean = p->k_mean; t->k_std = p->k_std;
+  size_t ng = p->gen_n.size();
+  if (t->gen_n) memcpy(t->gen_n, p->gen_n.data(), ng * 8);
+  if (t->gen_m) memcpy(t->gen_m, p->gen_m.data(), ng * 8);
+  if (t->gen_p) memcpy(t->gen_p, p->gen_p.data(), ng * 8);
+  if (t->gen_pc) memcpy(t->gen_pc, p->gen_pc.data(), ng * 8);
+  if (t->gen_k) memcpy(t->gen_k, p->gen_k.data(), ng * 8);
+  return TDR_OK;
+}
+
+int tdr_read_diagnostics(const tdr_problem *p, tdr_diag *o) {
+  if (!p || !o) return fail(TDR_EINVAL, "null argument");
+  *o = p->diag;
+  return TDR_OK;
+}
+
+int tdr_dev_det_log(const double *x, double *out, uint64_t n, void *stream) {
+  k_det_log<<<296, 256, 0, (cudaStream_t)stream>>>(x, out, n);
+  CK(cudaGetLastError()); CK(cudaStreamSynchronize((cudaStream_t)stream));
+  return TDR_OK;
+}
+int tdr_dev_draw(uint64_t seed, const uint64_t *id, uint32_t gen, uint32_t seg, uint32_t purpose, uint32_t j, double *out, uint64_t n, void *stream) {
+  k_draw<<<296, 256, 0, (cudaStream_t)stream>>>(seed, (const u64 *)id, gen, seg, purpose, j, out, n);
+  CK(cudaGetLastError()); CK(cudaStreamSynchronize((cudaStream_t)stream));
+  return TDR_OK;
+}

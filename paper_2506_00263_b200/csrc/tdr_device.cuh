@@ -1,0 +1,261 @@
+// tdr_device.cuh — device primitives and per-event physics (sm_100a, fp64, -fmad=false).
+// Follows DESIGN.md section 3 (N numerics, R RNG keying, G geometry, X cross sections, B birth,
+// T transport segment).  Shares nothing with oracle/.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+#include "../../include/tdr.h"
+
+#define TDR_INF __longlong_as_double(0x7FF0000000000000LL)
+#define FULL 0xFFFFFFFFu
+
+enum { PUR_DIST = 0, PUR_SELECT = 1, PUR_ENERGY = 2, PUR_DIR = 3, PUR_MULT = 4, PUR_POS = 5, PUR_POPCTRL = 6,
+       PUR_IDDERIVE = 15 };
+#define MAX_ATTEMPT 1024
+
+typedef unsigned long long u64;
+typedef long long i64;
+typedef unsigned int u32;
+
+// ---------------------------------------------------------------------------------- problem on the device
+struct DevProb {
+  int nx, ny, nz, n_univ, G, n_mat, n_e, by_group, n_grid, n_nuc;
+  int bc[6], mesh_n[3];
+  const double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges;
+  const int *cell_univ, *univ_nr, *univ_mat;
+  int src_kind, src_dir_kind, src_energy_kind, src_index;
+  double src_lo[3], src_hi[3], src_dir[3], src_energy, scale;
+  // MG table (staged to shared memory): per (m,g) row of MGROW doubles, then chi cdf per material
+  const double *mg; int mg_doubles;
+  // CE
+  const int *mat_nnuc, *mat_nuc; const double *mat_dens;
+  const double *grid; const double4 *xs;     // xs[nuc*n_grid + i] = {sig_s, sig_c, sig_f, 0}
+  const double *A, *nuc_nu, *wa, *wb;
+  const u32 *hash; u32 hash_bmin, hash_n;    // X3: bucket -> first candidate grid index
+  double grid_lo, grid_hi;
+  u64 n_bins;
+};
+// MG row layout: [0] sig_t [1] sig_s_tot [2] sig_c [3] nu*sig_f [4] nu [5..5+G) scatter cdf
+#define MGROW(G) (5 + (G))
+
+struct DevOut {
+  u64 *flux, *coll, *leak, *totals, *PPc;    // PPc[0] = P, PPc[1] = Pc
+  int *err;
+};
+
+struct Soa {                                  // particle state, one array per field
+  double *x, *y, *z, *u, *v, *w, *E;
+  u64 *id, *loc0, *loc1;
+  u32 *seg, *ncoll;
+  double *s_sigt, *s_nsf, *s_d, *s_f;        // split-decomposition scratch
+  u32 *s_flags, *s_gi;
+};
+
+struct DevRun {
+  u64 seed; u32 gen; int kmode, active; double k_prev;
+  int src_sites; const tdr_site *sites; u64 src_total; u64 *src_next;
+  tdr_site *sec; u64 sec_cap; u64 *sec_tail, *sec_head; u64 sec_limit, sec_head0;   // fixed-source secondaries (ring):
+                                                  // records [sec_head0, sec_limit) are complete and claimable
+  tdr_site *bank; u64 bank_cap; u64 *bank_count;                        // k-mode fission bank
+  u64 *hist_id; u32 *hist_nseg, *hist_ncoll; u64 *hist_count; u64 hist_cap;
+};
+
+struct Part {
+  double x, y, z, u, v, w, E;
+  u64 id;
+  int ix, iy, iz, ring, depth, mx, my, mz, g;
+  u32 seg, ncoll;
+};
+
+// ---------------------------------------------------------------------------------- R1 Philox4x32-10
+struct Blk { u32 w0, w1, w2, w3; };
+
+__device__ __forceinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {
+#pragma unroll
+  for (int r = 0; r < 10; r++) {
+    u32 h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+    u32 h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+    c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+    k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+  }
+  Blk b; b.w0 = c0; b.w1 = c1; b.w2 = c2; b.w3 = c3;
+  return b;
+}
+
+__device__ __forceinline__ Blk rng_block(u64 seed, u64 id, u32 gen, u32 seg, u32 purpose, u32 pair) {
+  u32 blk = (purpose << 12) | (pair & 0xFFFu);
+  return philox((u32)id, (u32)(id >> 32), (gen & 0xFFFFu) | (blk << 16), seg, (u32)seed, (u32)(seed >> 32));
+}
+
+__device__ __forceinline__ double to_unit(u32 lo, u32 hi) {          // N3
+  u64 u52 = (((u64)hi << 32) | lo) >> 12;
+  return (double)(i64)(2 * u52 + 1) * 0x1p-53;
+}
+__device__ __forceinline__ double blk_even(const Blk &b) { return to_unit(b.w0, b.w1); }
+__device__ __forceinline__ double blk_odd(const Blk &b) { return to_unit(b.w2, b.w3); }
+
+__device__ __forceinline__ double draw(u64 seed, u64 id, u32 gen, u32 seg, u32 purpose, u32 j) {
+  Blk b = rng_block(seed, id, gen, seg, purpose, j >> 1);
+  return (j & 1u) ? blk_odd(b) : blk_even(b);
+}
+
+__device__ __forceinline__ u64 derive_id(u64 seed, u64 id, u32 gen, u32 seg, u32 tag) {   // R4
+  Blk b = rng_block(seed, id, gen, seg, PUR_IDDERIVE, tag);
+  return ((u64)b.w1 << 32) | b.w0;
+}
+
+// ---------------------------------------------------------------------------------- N4 det_log
+__device__ __forceinline__ double det_log(double x) {
+  u64 bits = (u64)__double_as_longlong(x);
+  int e = (int)((bits >> 52) & 0x7FF) - 1022;
+  double m = __longlong_as_double((i64)((bits & 0x000FFFFFFFFFFFFFull) | 0x3FE0000000000000ull));
+  if (m < 0x1.6a09e667f3bcdp-1) { m = 2.0 * m; e = e - 1; }
+  double f = m - 1.0;
+  double s = f / (2.0 + f);
+  double z = s * s;
+  double p = 1.0 / 21.0;
+  p = __fma_rn(p, z, 1.0 / 19.0); p = __fma_rn(p, z, 1.0 / 17.0); p = __fma_rn(p, z, 1.0 / 15.0);
+  p = __fma_rn(p, z, 1.0 / 13.0); p = __fma_rn(p, z, 1.0 / 11.0); p = __fma_rn(p, z, 1.0 / 9.0);
+  p = __fma_rn(p, z, 1.0 / 7.0);  p = __fma_rn(p, z, 1.0 / 5.0);  p = __fma_rn(p, z, 1.0 / 3.0);
+  double t = (s * z) * p;
+  double r = 2.0 * (s + t);
+  double de = (double)e;
+  return (de * 0x1.62e42fee00000p-1) + ((de * 0x1.a39ef35793c76p-33) + r);
+}
+
+__device__ __forceinline__ i64 fixp(double v, double scale) { return __double2ll_rn(v * scale); }   // N5
+
+// ---------------------------------------------------------------------------------- B2 / B3 / T6 samplers
+__device__ __forceinline__ int iso_dir(u64 seed, u64 id, u32 gen, u32 seg, double &u, double &v, double &w) {
+  for (u32 a = 0; a < MAX_ATTEMPT; a++) {
+    Blk b = rng_block(seed, id, gen, seg, PUR_DIR, a);
+    double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;
+    double s = v1 * v1 + v2 * v2;
+    if (s < 1.0) {
+      double t = 2.0 * sqrt(1.0 - s);
+      u = v1 * t; v = v2 * t; w = 1.0 - 2.0 * s;
+      return 0;
+    }
+  }
+  u = 0.0; v = 0.0; w = 1.0;
+  return 1;
+}
+
+__device__ __forceinline__ double watt(u64 seed, u64 id, u32 gen, double a, double b) {
+  double cos2 = 1.0;
+  for (u32 t = 0; t < MAX_ATTEMPT; t++) {
+    Blk k = rng_block(seed, id, gen, 0, PUR_ENERGY, 4 + t);          // j = 8+2t, 9+2t
+    double v1 = 2.0 * blk_even(k) - 1.0, v2 = 2.0 * blk_odd(k) - 1.0;
+    double s = v1 * v1 + v2 * v2;
+    if (s < 1.0 && s > 0.0) { cos2 = (v1 * v1) / s; break; }
+  }
+  Blk b0 = rng_block(seed, id, gen, 0, PUR_ENERGY, 0), b1 = rng_block(seed, id, gen, 0, PUR_ENERGY, 1);
+  double l0 = det_log(blk_even(b0)), l1 = det_log(blk_odd(b0)), x2 = blk_even(b1);
+  double W = -a * (l0 + l1 * cos2);
+  double aab = (a * a) * b;
+  return (W + aab / 4.0) + (2.0 * x2 - 1.0) * sqrt(aab * W);
+}
+
+__device__ __forceinline__ void scatter_ce(u64 seed, u32 gen, Part &p, double A) {
+  double u = p.u, v = p.v, w = p.w;
+  double mu = 2.0 * draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0) - 1.0;
+  double q = (A * A + (2.0 * A) * mu) + 1.0;
+  p.E = p.E * (q / ((A + 1.0) * (A + 1.0)));
+  double mul = (1.0 + A * mu) / sqrt(q);
+  double cphi = 1.0, sphi = 0.0;
+  for (u32 t = 0; t < MAX_ATTEMPT; t++) {
+    Blk b = rng_block(seed, p.id, gen, p.seg, PUR_DIR, t);
+    double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;
+    double s = v1 * v1 + v2 * v2;
+    if (s < 1.0 && s > 0.0) { cphi = (v1 * v1 - v2 * v2) / s; sphi = (2.0 * v1 * v2) / s; break; }
+  }
+  double om = 1.0 - mul * mul; if (om < 0.0) om = 0.0;
+  double ow = 1.0 - w * w;
+  double un, vn, wn;
+  if (ow > 1e-10) {
+    double k = sqrt(om / ow);
+    un = mul * u + k * ((u * w) * cphi - v * sphi);
+    vn = mul * v + k * ((v * w) * cphi + u * sphi);
+    wn = mul * w - (k * ow) * cphi;
+  } else {
+    double k = sqrt(om);
+    un = k * cphi; vn = k * sphi; wn = (w > 0.0) ? mul : -mul;
+  }
+  double n = sqrt((un * un + vn * vn) + wn * wn);
+  p.u = un / n; p.v = vn / n; p.w = wn / n;
+}
+
+// ---------------------------------------------------------------------------------- G3 / G4 distances
+__device__ __forceinline__ double plane_dist(double lo, double hi, double x, double c) {
+  if (c > 0.0) return (hi - x) / c;
+  if (c < 0.0) return (lo - x) / c;
+  return TDR_INF;
+}
+
+__device__ __forceinline__ double dist_cyl(double X, double Y, double u, double v, double R, bool inside) {
+  double a = u * u + v * v;
+  if (a == 0.0) return TDR_INF;
+  double b = X * u + Y * v;
+  double c = (X * X + Y * Y) - R * R;
+  double disc = b * b - a * c;
+  double d;
+  if (inside) {
+    if (disc < 0.0) disc = 0.0;
+    d = (-b + sqrt(disc)) / a;
+  } else {
+    if (b >= 0.0) return TDR_INF;
+    if (disc <= 0.0) return TDR_INF;
+    d = (-b - sqrt(disc)) / a;
+  }
+  if (d < 0.0) d = 0.0;
+  return d;
+}
+
+__device__ __forceinline__ int find_bin(const double *pl, int n, double x) {   // G2
+  int k = 0;
+  for (int i = 1; i < n; i++) if (pl[i] <= x) k = i;
+  return k;
+}
+
+__device__ __forceinline__ int locate_ring(const DevProb &P, int univ, double X, double Y) {
+  int nr = P.univ_nr[univ];
+  double r2 = X * X + Y * Y;
+  for (int r = 0; r < nr; r++) { double R = P.univ_rad[univ * TDR_MAX_RINGS + r]; if (r2 < R * R) return r; }
+  return nr;
+}
+
+__device__ __forceinline__ int sample_cdf(const double *cdf, int n, double xi) {   // X1
+  double t = xi * cdf[n - 1];
+  for (int k = 0; k < n; k++) if (t < cdf[k]) return k;
+  return n - 1;
+}
+
+// ---------------------------------------------------------------------------------- SoA load / store
+__device__ __forceinline__ void unpack_loc(Part &p, u64 l0, u64 l1) {
+  p.ix = (int)(short)(l0 & 0xFFFF); p.iy = (int)(short)((l0 >> 16) & 0xFFFF); p.iz = (int)(short)((l0 >> 32) & 0xFFFF);
+  p.ring = (int)((l0 >> 48) & 0xFF); p.depth = (int)((l0 >> 56) & 0xFF);
+  p.mx = (int)(short)(l1 & 0xFFFF); p.my = (int)(short)((l1 >> 16) & 0xFFFF); p.mz = (int)(short)((l1 >> 32) & 0xFFFF);
+  p.g = (int)((l1 >> 48) & 0xFF);
+}
+__device__ __forceinline__ u64 pack_loc0(const Part &p) {
+  return (u64)(p.ix & 0xFFFF) | ((u64)(p.iy & 0xFFFF) << 16) | ((u64)(p.iz & 0xFFFF) << 32) |
+         ((u64)(p.ring & 0xFF) << 48) | ((u64)(p.depth & 0xFF) << 56);
+}
+__device__ __forceinline__ u64 pack_loc1(const Part &p) {
+  return (u64)(p.mx & 0xFFFF) | ((u64)(p.my & 0xFFFF) << 16) | ((u64)(p.mz & 0xFFFF) << 32) | ((u64)(p.g & 0xFF) << 48);
+}
+
+template <bool CE>
+__device__ __forceinline__ void load_part(const Soa &s, u32 i, Part &p) {
+  p.x = s.x[i]; p.y = s.y[i]; p.z = s.z[i]; p.u = s.u[i]; p.v = s.v[i]; p.w = s.w[i];
+  p.E = CE ? s.E[i] : 0.0;
+  p.id = s.id[i]; p.seg = s.seg[i]; p.ncoll = s.ncoll[i];
+  unpack_loc(p, s.loc0[i], s.loc1[i]);
+}
+template <bool CE>
+__device__ __forceinline__ void store_part(const Soa &s, u32 i, const Part &p) {
+  s.x[i] = p.x; s.y[i] = p.y; s.z[i] = p.z; s.u[i] = p.u; s.v[i] = p.v; s.w[i] = p.w;
+  if (CE) s.E[i] = p.E;
+  s.id[i] = p.id; s.seg[i] = p.seg; s.ncoll[i] = p.ncoll;
+  s.loc0[i] = pack_loc0(p); s.loc1[i] = pack_loc1(p);
+}

@@ -1,0 +1,300 @@
+// tdr_events.cuh — the transport events (A1-A6 of DESIGN.md section 2) on a register-resident particle.
+// LOOKUP (T1) -> MOVE (T2-T4) -> TALLY (T5) -> COLLIDE (T6) | SURFACE (T7); fused `step` = all of them
+// (monolithic task scheme), split = one kernel/event each (decomposed).
+#pragma once
+#include "tdr_device.cuh"
+
+// flags produced by MOVE
+enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512 };
+
+// per-block accumulators in shared memory, flushed once per kernel (finalize hook)
+struct BlockAcc {
+  u64 t64[TDR_T_COUNT];     // totals (nseg/ncoll/digest/nsites use 64-bit; others small)
+  u32 leak[6];
+  i64 P, Pc;
+};
+
+__device__ __forceinline__ void acc_init(BlockAcc *a) {
+  for (int i = threadIdx.x; i < (int)(sizeof(BlockAcc) / 4); i += blockDim.x) ((u32 *)a)[i] = 0;
+  __syncthreads();
+}
+
+__device__ __forceinline__ i64 warp_sum_i64(i64 v) {      // exact: 3 limbs of <= 24 bits via REDUX
+  u64 x = (u64)v;
+  u32 a = __reduce_add_sync(FULL, (u32)(x & 0xFFFFFFu));
+  u32 b = __reduce_add_sync(FULL, (u32)((x >> 24) & 0xFFFFFFu));
+  u32 c = __reduce_add_sync(FULL, (u32)(x >> 48));
+  return (i64)((u64)a + ((u64)b << 24) + ((u64)c << 48));
+}
+
+__device__ __forceinline__ void acc_flush(BlockAcc *a, const DevOut &o, i64 P, i64 Pc) {
+  i64 wp = warp_sum_i64(P), wpc = warp_sum_i64(Pc);      // two's complement limbs: exact mod 2^64
+  if ((threadIdx.x & 31) == 0) { atomicAdd((u64 *)&a->P, (u64)wp); atomicAdd((u64 *)&a->Pc, (u64)wpc); }
+  __syncthreads();
+  int t = threadIdx.x;
+  if (t < TDR_T_COUNT) { if (a->t64[t]) atomicAdd(&o.totals[t], a->t64[t]); }
+  else if (t < TDR_T_COUNT + 6) { if (a->leak[t - TDR_T_COUNT]) atomicAdd(&o.leak[t - TDR_T_COUNT], (u64)a->leak[t - TDR_T_COUNT]); }
+  else if (t == TDR_T_COUNT + 6) { if (a->P) atomicAdd(&o.PPc[0], (u64)a->P); }
+  else if (t == TDR_T_COUNT + 7) { if (a->Pc) atomicAdd(&o.PPc[1], (u64)a->Pc); }
+}
+
+// warp-cooperative tally: every lane of the warp calls it (valid = lane has a score)
+__device__ __forceinline__ void tally_add(u64 *arr, u64 bin, i64 val, bool valid) {
+  u32 m = __ballot_sync(FULL, valid);
+  if (m == 0) return;
+  int leader = __ffs(m) - 1;
+  u64 b0 = __shfl_sync(FULL, bin, leader);
+  bool same = __all_sync(FULL, !valid || bin == b0);
+  if (same) {
+    i64 s = warp_sum_i64(valid ? val : 0);
+    if ((threadIdx.x & 31) == leader) atomicAdd(&arr[b0], (u64)s);
+  } else if (valid) {
+    atomicAdd(&arr[bin], (u64)val);
+  }
+}
+
+// ---------------------------------------------------------------------------------- helpers
+__device__ __forceinline__ int cell_material(const DevProb &P, const Part &p, int &univ) {
+  univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+  return P.univ_mat[univ * (TDR_MAX_RINGS + 1) + p.ring];
+}
+
+__device__ __forceinline__ int grid_index(const DevProb &P, double El) {   // X3 hashed search == X2 index
+  u32 b = (u32)((u64)__double_as_longlong(El) >> 45) - P.hash_bmin;
+  u32 lo = P.hash[b], hi = P.hash[b + 1] + 1;       // grid[lo] <= El (or lo == 0), answer in [lo, hi)
+  if (hi > (u32)P.n_grid) hi = (u32)P.n_grid;
+  while (hi - lo > 1) {
+    u32 mid = lo + ((hi - lo) >> 1);
+    if (P.grid[mid] <= El) lo = mid; else hi = mid;
+  }
+  if (lo > (u32)P.n_grid - 2) lo = (u32)P.n_grid - 2;
+  return (int)lo;
+}
+
+// ---------------------------------------------------------------------------------- T1 LOOKUP
+template <bool CE>
+__device__ __forceinline__ void ev_lookup(const DevProb &P, const double *mg, const Part &p, double &St, double &nsf,
+                                          int &gi, double &f) {
+  int univ; int mat = cell_material(P, p, univ);
+  if (!CE) {
+    const double *row = mg + (mat * P.G + p.g) * MGROW(P.G);
+    St = row[0]; nsf = row[3]; gi = 0; f = 0.0;
+  } else {
+    double El = p.E; if (El < P.grid_lo) El = P.grid_lo; if (El > P.grid_hi) El = P.grid_hi;
+    gi = grid_index(P, El);
+    double e0 = P.grid[gi], e1 = P.grid[gi + 1];
+    f = (El - e0) / (e1 - e0);
+    St = 0.0; nsf = 0.0;
+    int nn = P.mat_nnuc[mat];
+    for (int n = 0; n < nn; n++) {
+      int nuc = P.mat_nuc[mat * TDR_MAX_NUC + n]; double N = P.mat_dens[mat * TDR_MAX_NUC + n];
+      const double4 a = P.xs[(size_t)nuc * P.n_grid + gi], b = P.xs[(size_t)nuc * P.n_grid + gi + 1];
+      double ss = a.x + f * (b.x - a.x), sc = a.y + f * (b.y - a.y), sf = a.z + f * (b.z - a.z);
+      double st = (ss + sc) + sf;
+      St = St + N * st;
+      nsf = nsf + N * (P.nuc_nu[nuc] * sf);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------- T2-T4 MOVE
+__device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Part &p, double St, double &d, u32 &flags) {
+  p.seg += 1;                                                          // R3
+  double dcoll = TDR_INF;
+  if (St > 0.0) dcoll = -det_log(draw(seed, p.id, gen, p.seg, PUR_DIST, 0)) / St;
+  double dx = plane_dist(P.xp[p.ix], P.xp[p.ix + 1], p.x, p.u);
+  double dy = plane_dist(P.yp[p.iy], P.yp[p.iy + 1], p.y, p.v);
+  double dz = plane_dist(P.zp[p.iz], P.zp[p.iz + 1], p.z, p.w);
+  double dout = TDR_INF, din = TDR_INF;
+  int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+  int nr = P.univ_nr[univ];
+  if (nr > 0) {
+    double X = p.x - P.cx[p.ix], Y = p.y - P.cy[p.iy];
+    if (p.ring < nr) dout = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring], true);
+    if (p.ring > 0) din = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring - 1], false);
+  }
+  double dmx = plane_dist(P.mesh[0][p.mx], P.mesh[0][p.mx + 1], p.x, p.u);
+  double dmy = plane_dist(P.mesh[1][p.my], P.mesh[1][p.my + 1], p.y, p.v);
+  double dmz = plane_dist(P.mesh[2][p.mz], P.mesh[2][p.mz + 1], p.z, p.w);
+  double ds = dx;
+  if (dy < ds) ds = dy;
+  if (dz < ds) ds = dz;
+  if (dout < ds) ds = dout;
+  if (din < ds) ds = din;
+  if (dmx < ds) ds = dmx;
+  if (dmy < ds) ds = dmy;
+  if (dmz < ds) ds = dmz;
+  bool collide = dcoll < ds;                                           // G5
+  d = collide ? dcoll : ds;
+  flags = 0;
+  if (!(d < TDR_INF)) { flags = F_LOST; d = 0.0; return; }
+  if (collide) flags = F_COLLIDE;
+  else flags = (dx == d ? F_DX : 0) | (dy == d ? F_DY : 0) | (dz == d ? F_DZ : 0) | (dout == d ? F_DOUT : 0) |
+               (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0);
+  p.x = p.x + d * p.u; p.y = p.y + d * p.v; p.z = p.z + d * p.w;       // G6
+}
+
+// ---------------------------------------------------------------------------------- T5 TALLY (warp-cooperative)
+template <bool CE>
+__device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, const DevRun &R, const Part &p, bool valid,
+                                         double d, double St, double nsf, u32 flags, i64 &accP, i64 &accPc) {
+  int e = -1;
+  if (valid) {
+    if (!CE) e = P.by_group ? p.g : 0;
+    else if (p.E >= P.e_edges[0] && p.E < P.e_edges[P.n_e]) {
+      int lo = 0, hi = P.n_e;
+      while (hi - lo > 1) { int mid = lo + ((hi - lo) >> 1); if (P.e_edges[mid] <= p.E) lo = mid; else hi = mid; }
+      e = lo;
+    }
+  }
+  bool collide = valid && (flags & F_COLLIDE);
+  if (R.kmode && valid) { accP += fixp(d * nsf, P.scale); if (collide) accPc += fixp(nsf / St, P.scale); }
+  if (R.active) {
+    u64 bin = 0;
+    if (e >= 0) bin = ((((u64)p.mz * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;
+    tally_add(o.flux, bin, fixp(d, P.scale), e >= 0);
+    tally_add(o.coll, bin, fixp(1.0, P.scale), e >= 0 && collide);
+  }
+}
+
+// ---------------------------------------------------------------------------------- death bookkeeping (D3)
+__device__ __forceinline__ void record_death(BlockAcc *a, const DevRun &R, const Part &p, int total_kind) {
+  atomicAdd(&a->t64[total_kind], 1ull);
+  atomicAdd(&a->t64[TDR_T_NSEG], (u64)p.seg);
+  atomicAdd(&a->t64[TDR_T_NCOLL], (u64)p.ncoll);
+  atomicAdd(&a->t64[TDR_T_NCROSS], (u64)(p.seg - p.ncoll));
+  Blk h = philox((u32)p.id, (u32)(p.id >> 32), p.ncoll, p.seg - p.ncoll, p.seg, 0x7D12u);
+  atomicAdd(&a->t64[TDR_T_DIGEST], ((u64)h.w1 << 32) | h.w0);
+  if (R.hist_cap) {
+    u64 k = atomicAdd(R.hist_count, 1ull);
+    if (k < R.hist_cap) { R.hist_id[k] = p.id; R.hist_nseg[k] = p.seg; R.hist_ncoll[k] = p.ncoll; }
+  }
+}
+
+// ---------------------------------------------------------------------------------- T6 COLLIDE
+// returns true if the particle survives; n_children / child_src set on fission
+template <bool CE>
+__device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
+                                           double St, int gi, double f, int &n_children, int &child_src) {
+  const u64 seed = R.seed; const u32 gen = R.gen;
+  n_children = 0; child_src = 0;
+  p.ncoll += 1;
+  int univ; int mat = cell_material(P, p, univ);
+  int kind; double nu;
+  if (!CE) {
+    const double *row = mg + (mat * P.G + p.g) * MGROW(P.G);
+    double r = draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * St;
+    if (r < row[1]) kind = 0; else if (r < row[1] + row[2]) kind = 1; else kind = 2;
+    nu = row[4]; child_src = mat;
+    if (kind == 0) {
+      p.g = sample_cdf(row + 5, P.G, draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0));
+      if (iso_dir(seed, p.id, gen, p.seg, p.u, p.v, p.w)) atomicAdd(&acc->t64[TDR_T_NDIRFAIL], 1ull);
+      return true;
+    }
+  } else {
+    Blk sb = rng_block(seed, p.id, gen, p.seg, PUR_SELECT, 0);
+    double r = blk_even(sb) * St;
+    int nn = P.mat_nnuc[mat];
+    double acc_s = 0.0, ss = 0.0, sc = 0.0, st = 0.0; int nuc = 0;
+    for (int n = 0; n < nn; n++) {
+      nuc = P.mat_nuc[mat * TDR_MAX_NUC + n]; double N = P.mat_dens[mat * TDR_MAX_NUC + n];
+      const double4 a = P.xs[(size_t)nuc * P.n_grid + gi], b = P.xs[(size_t)nuc * P.n_grid + gi + 1];
+      ss = a.x + f * (b.x - a.x); sc = a.y + f * (b.y - a.y); double sf = a.z + f * (b.z - a.z);
+      st = (ss + sc) + sf;
+      acc_s = acc_s + N * st;
+      if (r < acc_s) break;
+    }
+    double r2 = blk_odd(sb) * st;
+    if (r2 < ss) kind = 0; else if (r2 < ss + sc) kind = 1; else kind = 2;
+    nu = P.nuc_nu[nuc]; child_src = nuc;
+    if (kind == 0) { scatter_ce(seed, gen, p, P.A[nuc]); return true; }
+  }
+  if (kind == 1) { record_death(acc, R, p, TDR_T_NABS); return false; }
+  double nu_eff = R.kmode ? nu / R.k_prev : nu;
+  int n = (int)floor(nu_eff + draw(seed, p.id, gen, p.seg, PUR_MULT, 0));
+  if (n > 64) n = 64;
+  if (!R.kmode && p.depth >= 200) { atomicAdd(&acc->t64[TDR_T_NDROPPED], (u64)n); n = 0; }
+  n_children = n;
+  record_death(acc, R, p, TDR_T_NFIS);
+  return false;
+}
+
+// ---------------------------------------------------------------------------------- T7 SURFACE (G7)
+__device__ __forceinline__ bool ev_surface(const DevProb &P, const DevRun &R, BlockAcc *acc, Part &p, u32 flags) {
+  bool alive = true;
+  const double u0 = p.u, v0 = p.v, w0 = p.w;
+  int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+  bool moved_xy = false, moved_z = false;
+  if (flags & F_DX) {
+    if (u0 > 0.0) { p.x = P.xp[p.ix + 1]; if (p.ix + 1 == P.nx) { if (P.bc[1]) p.u = -u0; else { alive = false; atomicAdd(&acc->leak[1], 1u); } } else { p.ix += 1; moved_xy = true; } }
+    else { p.x = P.xp[p.ix]; if (p.ix == 0) { if (P.bc[0]) p.u = -u0; else { alive = false; atomicAdd(&acc->leak[0], 1u); } } else { p.ix -= 1; moved_xy = true; } }
+  }
+  if (flags & F_DY) {
+    if (v0 > 0.0) { p.y = P.yp[p.iy + 1]; if (p.iy + 1 == P.ny) { if (P.bc[3]) p.v = -v0; else { alive = false; atomicAdd(&acc->leak[3], 1u); } } else { p.iy += 1; moved_xy = true; } }
+    else { p.y = P.yp[p.iy]; if (p.iy == 0) { if (P.bc[2]) p.v = -v0; else { alive = false; atomicAdd(&acc->leak[2], 1u); } } else { p.iy -= 1; moved_xy = true; } }
+  }
+  if (flags & F_DZ) {
+    if (w0 > 0.0) { p.z = P.zp[p.iz + 1]; if (p.iz + 1 == P.nz) { if (P.bc[5]) p.w = -w0; else { alive = false; atomicAdd(&acc->leak[5], 1u); } } else { p.iz += 1; moved_z = true; } }
+    else { p.z = P.zp[p.iz]; if (p.iz == 0) { if (P.bc[4]) p.w = -w0; else { alive = false; atomicAdd(&acc->leak[4], 1u); } } else { p.iz -= 1; moved_z = true; } }
+  }
+  if (flags & F_DOUT) p.ring += 1;
+  if (flags & F_DIN) p.ring -= 1;
+  if (moved_xy || moved_z) {
+    int nu2 = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+    if (moved_xy) p.ring = P.univ_nr[nu2];
+    else if (nu2 != univ) p.ring = locate_ring(P, nu2, p.x - P.cx[p.ix], p.y - P.cy[p.iy]);
+  }
+  if (flags & F_MX) { if (u0 > 0.0) { p.x = P.mesh[0][p.mx + 1]; if (p.mx + 1 < P.mesh_n[0]) p.mx += 1; } else { p.x = P.mesh[0][p.mx]; if (p.mx > 0) p.mx -= 1; } }
+  if (flags & F_MY) { if (v0 > 0.0) { p.y = P.mesh[1][p.my + 1]; if (p.my + 1 < P.mesh_n[1]) p.my += 1; } else { p.y = P.mesh[1][p.my]; if (p.my > 0) p.my -= 1; } }
+  if (flags & F_MZ) { if (w0 > 0.0) { p.z = P.mesh[2][p.mz + 1]; if (p.mz + 1 < P.mesh_n[2]) p.mz += 1; } else { p.z = P.mesh[2][p.mz]; if (p.mz > 0) p.mz -= 1; } }
+  if (!alive) record_death(acc, R, p, TDR_T_NLEAK);
+  return alive;
+}
+
+// ---------------------------------------------------------------------------------- B birth (A1 SOURCE)
+template <bool CE>
+__device__ __forceinline__ void birth_common(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
+                                             int src, bool from_site) {
+  p.seg = 0; p.ncoll = 0; p.E = 0.0; p.g = 0;
+  if (!from_site && P.src_dir_kind == 1) { p.u = P.src_dir[0]; p.v = P.src_dir[1]; p.w = P.src_dir[2]; }
+  else if (iso_dir(R.seed, p.id, R.gen, 0, p.u, p.v, p.w)) atomicAdd(&acc->t64[TDR_T_NDIRFAIL], 1ull);
+  if (from_site) {
+    if (!CE) p.g = sample_cdf(mg + P.n_mat * P.G * MGROW(P.G) + src * P.G, P.G, draw(R.seed, p.id, R.gen, 0, PUR_ENERGY, 0));
+    else p.E = watt(R.seed, p.id, R.gen, P.wa[src], P.wb[src]);
+  } else if (P.src_energy_kind == 0) p.g = P.src_index;
+  else if (P.src_energy_kind == 1) p.E = P.src_energy;
+  else p.E = watt(R.seed, p.id, R.gen, P.wa[P.src_index], P.wb[P.src_index]);
+  atomicAdd(&acc->t64[TDR_T_NBORN], 1ull);
+}
+
+template <bool CE>
+__device__ __forceinline__ void birth_primary(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, u64 i) {
+  p.id = i; p.depth = 0;
+  if (P.src_kind == 0) { p.x = P.src_lo[0]; p.y = P.src_lo[1]; p.z = P.src_lo[2]; }
+  else {
+    Blk b0 = rng_block(R.seed, i, R.gen, 0, PUR_POS, 0), b1 = rng_block(R.seed, i, R.gen, 0, PUR_POS, 1);
+    p.x = P.src_lo[0] + blk_even(b0) * (P.src_hi[0] - P.src_lo[0]);
+    p.y = P.src_lo[1] + blk_odd(b0) * (P.src_hi[1] - P.src_lo[1]);
+    p.z = P.src_lo[2] + blk_even(b1) * (P.src_hi[2] - P.src_lo[2]);
+  }
+  p.ix = find_bin(P.xp, P.nx, p.x); p.iy = find_bin(P.yp, P.ny, p.y); p.iz = find_bin(P.zp, P.nz, p.z);
+  p.mx = find_bin(P.mesh[0], P.mesh_n[0], p.x); p.my = find_bin(P.mesh[1], P.mesh_n[1], p.y); p.mz = find_bin(P.mesh[2], P.mesh_n[2], p.z);
+  int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+  p.ring = locate_ring(P, univ, p.x - P.cx[p.ix], p.y - P.cy[p.iy]);
+  birth_common<CE>(P, mg, R, acc, p, 0, false);
+}
+
+template <bool CE>
+__device__ __forceinline__ void birth_site(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, const tdr_site &s) {
+  p.id = s.id; p.depth = s.depth; p.x = s.x; p.y = s.y; p.z = s.z;
+  p.ix = s.ix; p.iy = s.iy; p.iz = s.iz; p.mx = s.mx; p.my = s.my; p.mz = s.mz; p.ring = s.ring;
+  birth_common<CE>(P, mg, R, acc, p, s.src, true);
+}
+
+__device__ __forceinline__ tdr_site make_site(const DevRun &R, const Part &p, int src, u32 c) {
+  tdr_site s;
+  s.x = p.x; s.y = p.y; s.z = p.z; s.id = derive_id(R.seed, p.id, R.gen, p.seg, c);
+  s.ix = (short)p.ix; s.iy = (short)p.iy; s.iz = (short)p.iz; s.mx = (short)p.mx; s.my = (short)p.my; s.mz = (short)p.mz;
+  s.ring = (unsigned char)p.ring; s.src = (unsigned char)src; s.depth = (unsigned char)(R.kmode ? 0 : p.depth + 1); s.pad = 0;
+  return s;
+}

@@ -1,0 +1,182 @@
+// tdr_stack.cuh — stack-based remapping: per-event particle-index stacks with device counters,
+// warp-collective push (one atomicAdd per warp, lanes index relative to it), pop by grid-stride over [0, count).
+// make_work is folded into the event that kills a particle: the dead lane claims the next
+// source index (or a pending secondary) with a warp-aggregated atomic and is reborn in the same slot.
+#pragma once
+#include "tdr_events.cuh"
+
+// device counters (u64 each), one 128-byte readback per remap iteration
+enum { C_SRC_NEXT = 0, C_SEC_TAIL, C_SEC_HEAD, C_BANK, C_HIST, C_NEXT_BANK, C_PENDING, C_STARVED,
+       C_STACK0 = 8, /* C_STACK0..+7: stack counts */ C_COUNT = 16 };
+
+// event ids (split decomposition; async scheme)
+enum { EV_LOOKUP = 0, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_STEP, EV_FREE, EV_COUNT };
+
+__device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
+
+// warp-collective push of one index per flagged lane
+__device__ __forceinline__ void stack_push(u32 *stack, u64 *count, u32 value, bool pred) {
+  u32 m = __ballot_sync(FULL, pred);
+  if (m == 0) return;
+  int leader = __ffs(m) - 1;
+  u64 base = 0;
+  if ((threadIdx.x & 31) == leader) base = atomicAdd(count, (u64)__popc(m));
+  base = __shfl_sync(FULL, base, leader);
+  if (pred) stack[base + __popc(m & lanemask_lt())] = value;
+}
+
+// warp-collective push of n sites per lane into the fission bank (k-mode) or the secondary ring (fixed source)
+__device__ __forceinline__ void push_children(const DevOut &O, const DevRun &R, BlockAcc *acc, const Part &p, int n, int src) {
+  u32 lane = threadIdx.x & 31;
+  u32 total = __reduce_add_sync(FULL, (u32)n);
+  if (total == 0) return;
+  u32 incl = (u32)n;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { u32 t = __shfl_up_sync(FULL, incl, o); if (lane >= (u32)o) incl += t; }
+  u32 excl = incl - (u32)n;
+  u64 base = 0;
+  if (lane == 0) { base = atomicAdd(R.kmode ? R.bank_count : R.sec_tail, (u64)total); atomicAdd(&acc->t64[TDR_T_NSITES], (u64)total); }
+  base = __shfl_sync(FULL, base, 0);
+  for (int c = 0; c < n; c++) {
+    u64 t = base + excl + c;
+    tdr_site s = make_site(R, p, src, (u32)c);
+    if (R.kmode) { if (t < R.bank_cap) R.bank[t] = s; else atomicExch(O.err, TDR_ECAPACITY); }
+    else { if (t - R.sec_head0 < R.sec_cap) R.sec[t % R.sec_cap] = s; else atomicExch(O.err, TDR_ECAPACITY); }
+  }
+}
+
+// make_work for dead lanes: pending secondaries first, then the primary source.  Returns true if reborn.
+template <bool CE>
+__device__ __forceinline__ bool make_work(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, bool dead) {
+  u32 lane = threadIdx.x & 31;
+  bool reborn = false;
+  if (!R.kmode && R.sec_limit > R.sec_head0) {
+    u32 m = __ballot_sync(FULL, dead);
+    if (m) {
+      int leader = __ffs(m) - 1; u64 h = ~0ull;
+      if (lane == (u32)leader && *(volatile u64 *)R.sec_head < R.sec_limit) h = atomicAdd(R.sec_head, (u64)__popc(m));
+      h = __shfl_sync(FULL, h, leader);
+      if (dead && h != ~0ull) {
+        u64 idx = h + __popc(m & lanemask_lt());
+        if (idx < R.sec_limit) { tdr_site s = R.sec[idx % R.sec_cap]; birth_site<CE>(P, mg, R, acc, p, s); reborn = true; }
+      }
+    }
+  }
+  u32 m = __ballot_sync(FULL, dead && !reborn);
+  if (m) {
+    int leader = __ffs(m) - 1; u64 h = ~0ull;
+    if (lane == (u32)leader && *(volatile u64 *)R.src_next < R.src_total) h = atomicAdd(R.src_next, (u64)__popc(m));
+    h = __shfl_sync(FULL, h, leader);
+    if (dead && !reborn && h != ~0ull) {
+      u64 idx = h + __popc(m & lanemask_lt());
+      if (idx < R.src_total) {
+        if (R.src_sites) { tdr_site s = R.sites[idx]; birth_site<CE>(P, mg, R, acc, p, s); }
+        else birth_primary<CE>(P, mg, R, acc, p, idx);
+        reborn = true;
+      }
+    }
+  }
+  return reborn;
+}
+
+__device__ __forceinline__ const double *stage_mg(const DevProb &P, double *smem) {
+  if (P.G == 0) return nullptr;
+  for (int i = threadIdx.x; i < P.mg_doubles; i += blockDim.x) smem[i] = P.mg[i];
+  return smem;
+}
+
+// ---------------------------------------------------------------------------------- A1 SOURCE: fill slots [0, n)
+template <bool CE>
+__global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, Soa S, u32 *stack, u64 *count,
+                                                u64 sec_start, u64 n_sec, u64 src_start, u64 n) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  acc_init(&acc);
+  for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
+    Part p;
+    if (i < n_sec) { tdr_site s = R.sec[(sec_start + i) % R.sec_cap]; birth_site<CE>(P, mg, R, &acc, p, s); }
+    else {
+      u64 idx = src_start + (i - n_sec);
+      if (R.src_sites) { tdr_site s = R.sites[idx]; birth_site<CE>(P, mg, R, &acc, p, s); }
+      else birth_primary<CE>(P, mg, R, &acc, p, idx);
+    }
+    store_part<CE>(S, (u32)i, p);
+    stack[i] = (u32)i;
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) *count = n;
+  acc_flush(&acc, O, 0, 0);
+}
+
+// ---------------------------------------------------------------------------------- fused STEP (monolithic scheme)
+template <bool CE>
+__global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in,
+                                              u32 *stack_out, u64 *count_out) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  acc_init(&acc);
+  const u64 n_in = *count_in;
+  i64 accP = 0, accPc = 0;
+  for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_in; i0 += (u64)gridDim.x * blockDim.x) {
+    u64 i = i0 + threadIdx.x;
+    bool valid = i < n_in;
+    Part p; u32 slot = 0;
+    double St = 0.0, nsf = 0.0, d = 0.0, f = 0.0; int gi = 0; u32 flags = 0;
+    if (valid) {
+      slot = stack_in[i];
+      load_part<CE>(S, slot, p);
+      ev_lookup<CE>(P, mg, p, St, nsf, gi, f);
+      ev_move(P, R.seed, R.gen, p, St, d, flags);
+    }
+    ev_tally<CE>(P, O, R, p, valid && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
+    bool alive = false; int nch = 0, csrc = 0;
+    if (valid) {
+      if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
+      else if (flags & F_COLLIDE) alive = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+      else alive = ev_surface(P, R, &acc, p, flags);
+    }
+    push_children(O, R, &acc, p, nch, csrc);
+    if (make_work<CE>(P, mg, R, &acc, p, valid && !alive)) alive = true;
+    if (alive) store_part<CE>(S, slot, p);
+    stack_push(stack_out, count_out, slot, alive);
+  }
+  acc_flush(&acc, O, accP, accPc);
+}
+
+// ---------------------------------------------------------------------------------- A9 population control (D2)
+__global__ void __launch_bounds__(256) k_popctrl(const tdr_site *bank, u64 n_bank, tdr_site *next, u64 next_cap, u64 *next_count,
+                                                 u64 seed, u32 gen_next, double pr, int *err) {
+  u32 lane = threadIdx.x & 31;
+  for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_bank; i0 += (u64)gridDim.x * blockDim.x) {
+    u64 i = i0 + threadIdx.x;
+    int m = 0; tdr_site s;
+    if (i < n_bank) {
+      s = bank[i];
+      m = (int)floor(pr + draw(seed, s.id, gen_next, 0, PUR_POPCTRL, 0));
+      if (m > 2048) m = 2048;
+    }
+    u32 total = __reduce_add_sync(FULL, (u32)m);
+    if (total == 0) continue;
+    u32 incl = (u32)m;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { u32 t = __shfl_up_sync(FULL, incl, o); if (lane >= (u32)o) incl += t; }
+    u64 base = 0;
+    if (lane == 0) base = atomicAdd(next_count, (u64)total);
+    base = __shfl_sync(FULL, base, 0) + (incl - (u32)m);
+    u64 sid = s.id;
+    for (int r = 0; r < m; r++) {
+      s.id = derive_id(seed, sid, gen_next, 0, 2048u + (u32)r);
+      if (base + r < next_cap) next[base + r] = s; else atomicExch(err, TDR_ECAPACITY);
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------- unit kernels
+__global__ void k_det_log(const double *x, double *out, u64 n) {
+  for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) out[i] = det_log(x[i]);
+}
+__global__ void k_draw(u64 seed, const u64 *id, u32 gen, u32 seg, u32 purpose, u32 j, double *out, u64 n) {
+  for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x)
+    out[i] = draw(seed, id[i], gen, seg, purpose, j);
+}

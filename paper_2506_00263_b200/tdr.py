@@ -1,0 +1,223 @@
+"""Thin ctypes binding of libtdr.so (include/tdr.h).  Argument marshalling only: every step of the
+transport path runs in the CUDA kernels.  torch supplies device memory (the workspace) and the stream.
+There is no CPU fallback: a missing library or device raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import build as _build
+
+MAX_RINGS, MAX_NUC, T_COUNT = 4, 4, 12
+TOTAL_NAMES = ["n_seg", "n_coll", "n_cross", "n_abs", "n_fis", "n_leak", "n_born", "n_dropped",
+               "n_dirfail", "digest", "n_sites"]
+SITE_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("id", "<u8"), ("ix", "<i2"), ("iy", "<i2"),
+                       ("iz", "<i2"), ("mx", "<i2"), ("my", "<i2"), ("mz", "<i2"), ("ring", "u1"),
+                       ("src", "u1"), ("depth", "u1"), ("pad", "u1")])
+PD, PI = C.POINTER(C.c_double), C.POINTER(C.c_int32)
+
+
+class tdr_geometry(C.Structure):
+    _fields_ = [("nx", C.c_int32), ("ny", C.c_int32), ("nz", C.c_int32),
+                ("xplanes", PD), ("yplanes", PD), ("zplanes", PD), ("cx", PD), ("cy", PD), ("cell_univ", PI),
+                ("bc", C.c_int32 * 6), ("n_univ", C.c_int32), ("univ_nrings", PI), ("univ_radius", PD), ("univ_mat", PI),
+                ("mesh_n", C.c_int32 * 3), ("mesh_x", PD), ("mesh_y", PD), ("mesh_z", PD),
+                ("by_group", C.c_int32), ("n_ebins", C.c_int32), ("e_edges", PD),
+                ("src_kind", C.c_int32), ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3),
+                ("src_dir_kind", C.c_int32), ("src_dir", C.c_double * 3),
+                ("src_energy_kind", C.c_int32), ("src_index", C.c_int32), ("src_energy", C.c_double),
+                ("tally_scale_log2", C.c_int32)]
+
+
+class tdr_materials(C.Structure):
+    _fields_ = [("n_mat", C.c_int32), ("G", C.c_int32), ("sig_t", PD), ("sig_s", PD), ("sig_f", PD), ("nu", PD),
+                ("chi", PD), ("mat_nnuc", PI), ("mat_nuc", PI), ("mat_dens", PD)]
+
+
+class tdr_xs_tables(C.Structure):
+    _fields_ = [("n_grid", C.c_int32), ("n_nuc", C.c_int32), ("energy", PD), ("A", PD), ("sig_s", PD), ("sig_c", PD),
+                ("sig_f", PD), ("nu", PD), ("watt_a", PD), ("watt_b", PD)]
+
+
+class tdr_sizes(C.Structure):
+    _fields_ = [("n_bins", C.c_uint64), ("n_gen", C.c_uint64), ("n_hist", C.c_uint64), ("n_bank", C.c_uint64)]
+
+
+class tdr_tallies(C.Structure):
+    _fields_ = [("flux", C.c_void_p), ("coll", C.c_void_p), ("leak", C.c_int64 * 6), ("totals", C.c_uint64 * T_COUNT),
+                ("k_mean", C.c_double), ("k_std", C.c_double), ("gen_n", C.c_void_p), ("gen_m", C.c_void_p),
+                ("gen_p", C.c_void_p), ("gen_pc", C.c_void_p), ("gen_k", C.c_void_p), ("hist_id", C.c_void_p),
+                ("hist_nseg", C.c_void_p), ("hist_ncoll", C.c_void_p), ("bank", C.c_void_p)]
+
+
+class tdr_diag(C.Structure):
+    _fields_ = [("kernel_launches", C.c_uint64), ("iterations", C.c_uint64), ("events", C.c_uint64 * 8),
+                ("spills", C.c_uint64), ("fetches", C.c_uint64), ("make_work_calls", C.c_uint64),
+                ("gpu_ms", C.c_double), ("step_ms", C.c_double), ("step_launches", C.c_uint64)]
+
+
+EXPORTS = ["tdr_init_problem", "tdr_set_option", "tdr_workspace_bytes", "tdr_bind_workspace", "tdr_run_fixed_source",
+           "tdr_run_k_eigenvalue", "tdr_tally_sizes", "tdr_read_tallies", "tdr_read_diagnostics", "tdr_free_problem",
+           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw"]
+
+_lib = None
+
+
+def lib():
+    """Load libtdr.so (building it in-tree if the sources are newer).  Raises if it cannot be loaded."""
+    global _lib
+    if _lib is None:
+        path = _build.build() if os.path.exists(_build.CSRC) else _build.LIB
+        L = C.CDLL(path)
+        L.tdr_init_problem.argtypes = [C.POINTER(tdr_geometry), C.POINTER(tdr_materials), C.POINTER(tdr_xs_tables), C.POINTER(C.c_void_p)]
+        L.tdr_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_char_p]
+        L.tdr_workspace_bytes.argtypes = [C.c_void_p, C.c_uint64, C.POINTER(C.c_uint64)]
+        L.tdr_bind_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+        L.tdr_run_fixed_source.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
+        L.tdr_run_k_eigenvalue.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint64]
+        L.tdr_tally_sizes.argtypes = [C.c_void_p, C.POINTER(tdr_sizes)]
+        L.tdr_read_tallies.argtypes = [C.c_void_p, C.POINTER(tdr_tallies)]
+        L.tdr_read_diagnostics.argtypes = [C.c_void_p, C.POINTER(tdr_diag)]
+        L.tdr_free_problem.argtypes = [C.c_void_p]
+        L.tdr_free_problem.restype = None
+        L.tdr_last_error.restype = C.c_char_p
+        L.tdr_dev_det_log.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
+        L.tdr_dev_draw.argtypes = [C.c_uint64, C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_uint64, C.c_void_p]
+        _lib = L
+    return _lib
+
+
+class TdrError(RuntimeError):
+    def __init__(self, code, what):
+        super().__init__(f"{what}: code {code}: {lib().tdr_last_error().decode()}")
+        self.code = code
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise TdrError(rc, what)
+
+
+def _fill(struct, d, keep):
+    for name, ctype in struct._fields_:
+        if name not in d:
+            continue
+        v = d[name]
+        if ctype is PD:
+            a = np.ascontiguousarray(v, dtype=np.float64); keep.append(a); setattr(struct, name, a.ctypes.data_as(PD))
+        elif ctype is PI:
+            a = np.ascontiguousarray(v, dtype=np.int32); keep.append(a); setattr(struct, name, a.ctypes.data_as(PI))
+        elif isinstance(v, (np.ndarray, list, tuple)):
+            setattr(struct, name, ctype(*[x.item() if hasattr(x, "item") else x for x in np.asarray(v).ravel()]))
+        else:
+            setattr(struct, name, v)
+    return struct
+
+
+class Problem:
+    """init_problem / run_fixed_source / run_k_eigenvalue / read_tallies on one CUDA device."""
+
+    def __init__(self, problem, device="cuda:0", **options):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2506_00263_b200 needs a CUDA device: there is no CPU fallback")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.problem = problem
+        keep = []
+        g = _fill(tdr_geometry(), problem.geometry, keep)
+        m = _fill(tdr_materials(), problem.materials, keep)
+        x = _fill(tdr_xs_tables(), problem.xs, keep) if problem.xs is not None else None
+        self.h = C.c_void_p()
+        _check(lib().tdr_init_problem(C.byref(g), C.byref(m), C.byref(x) if x is not None else None, C.byref(self.h)), "tdr_init_problem")
+        self.ws = None
+        for k, v in options.items():
+            self.set_option(k, v)
+
+    def set_option(self, key, value):
+        _check(lib().tdr_set_option(self.h, str(key).encode(), str(value).encode()), f"tdr_set_option({key})")
+
+    def _bind(self, n):
+        need = C.c_uint64()
+        _check(lib().tdr_workspace_bytes(self.h, n, C.byref(need)), "tdr_workspace_bytes")
+        if self.ws is None or self.ws.numel() < need.value:
+            self.ws = None
+            self.ws = self.torch.empty(need.value + 256, dtype=self.torch.uint8, device=self.device)
+        ptr = (self.ws.data_ptr() + 255) & ~255
+        stream = self.torch.cuda.current_stream(self.device).cuda_stream
+        _check(lib().tdr_bind_workspace(self.h, ptr, need.value, stream), "tdr_bind_workspace")
+
+    def run_fixed_source(self, n_particles, seed):
+        self._bind(n_particles)
+        _check(lib().tdr_run_fixed_source(self.h, n_particles, seed), "tdr_run_fixed_source")
+
+    def run_k_eigenvalue(self, n_particles, n_inactive, n_active, seed):
+        self._bind(n_particles)
+        _check(lib().tdr_run_k_eigenvalue(self.h, n_particles, n_inactive, n_active, seed), "tdr_run_k_eigenvalue")
+
+    def run(self, n=None, n_inactive=None, n_active=None, seed=None):
+        p = self.problem
+        n = p.n_particles if n is None else n
+        seed = p.seed if seed is None else seed
+        if p.mode == "fixed":
+            self.run_fixed_source(n, seed)
+        else:
+            self.run_k_eigenvalue(n, p.n_inactive if n_inactive is None else n_inactive,
+                                  p.n_active if n_active is None else n_active, seed)
+        return self.read_tallies()
+
+    def read_tallies(self, history=True, bank=True):
+        s = tdr_sizes()
+        _check(lib().tdr_tally_sizes(self.h, C.byref(s)), "tdr_tally_sizes")
+        out = dict(flux=np.zeros(s.n_bins, np.int64), coll=np.zeros(s.n_bins, np.int64),
+                   gen_n=np.zeros(s.n_gen, np.uint64), gen_m=np.zeros(s.n_gen, np.uint64),
+                   gen_p=np.zeros(s.n_gen, np.int64), gen_pc=np.zeros(s.n_gen, np.int64), gen_k=np.zeros(s.n_gen, np.float64))
+        if history:
+            out.update(hist_id=np.zeros(s.n_hist, np.uint64), hist_nseg=np.zeros(s.n_hist, np.uint32), hist_ncoll=np.zeros(s.n_hist, np.uint32))
+        if bank:
+            out.update(bank=np.zeros(s.n_bank, SITE_DTYPE))
+        t = tdr_tallies()
+        for k, a in out.items():
+            setattr(t, k, a.ctypes.data)
+        _check(lib().tdr_read_tallies(self.h, C.byref(t)), "tdr_read_tallies")
+        out["leak"] = np.array(list(t.leak), np.int64)
+        out["totals"] = {n: int(t.totals[i]) for i, n in enumerate(TOTAL_NAMES)}
+        out["k_mean"], out["k_std"] = t.k_mean, t.k_std
+        return out
+
+    def diagnostics(self):
+        d = tdr_diag()
+        _check(lib().tdr_read_diagnostics(self.h, C.byref(d)), "tdr_read_diagnostics")
+        return dict(kernel_launches=d.kernel_launches, iterations=d.iterations, events=list(d.events), spills=d.spills,
+                    fetches=d.fetches, make_work_calls=d.make_work_calls, gpu_ms=d.gpu_ms, step_ms=d.step_ms,
+                    step_launches=d.step_launches)
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib().tdr_free_problem(self.h)
+            self.h = C.c_void_p()
+        self.ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def dev_det_log(x):
+    """x: torch cuda float64 tensor -> det_log(x) computed by the device primitive."""
+    import torch
+    out = torch.empty_like(x)
+    _check(lib().tdr_dev_det_log(x.data_ptr(), out.data_ptr(), x.numel(), torch.cuda.current_stream().cuda_stream), "tdr_dev_det_log")
+    return out
+
+
+def dev_draw(seed, ids, gen, seg, purpose, j):
+    import torch
+    out = torch.empty(ids.numel(), dtype=torch.float64, device=ids.device)
+    _check(lib().tdr_dev_draw(seed, ids.data_ptr(), gen, seg, purpose, j, out.data_ptr(), ids.numel(), torch.cuda.current_stream().cuda_stream), "tdr_dev_draw")
+    return out

@@ -206,7 +206,7 @@ def cfg2(n=10000000, n_inactive=6, n_active=18, seed=1):
 
 
 # --------------------------------------------------------------------------- continuous energy
-def ce_tables(n_grid=50000, n_res=200, sigf0=2.5, seed=PROBLEM_SEED):
+def ce_tables(n_grid=50000, n_res=200, sigf0=2.5, res_fis=0.05, seed=PROBLEM_SEED):
     """3 synthetic nuclides (A=1,16,238) on a log grid 1e-5 eV .. 2e7 eV."""
     rng = np.random.default_rng(seed + 1)
     E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
@@ -228,15 +228,15 @@ def ce_tables(n_grid=50000, n_res=200, sigf0=2.5, seed=PROBLEM_SEED):
         s[2] = s[2] + s0 * (gn / gt) * lor
         cap = s0 * (gg / gt) * np.sqrt(Er / E) * lor
         c[2] = c[2] + cap
-        f[2] = f[2] + 0.05 * cap
+        f[2] = f[2] + res_fis * cap
     return dict(n_grid=n_grid, n_nuc=3, energy=_f64(E), A=_f64([1.0, 16.0, 238.0]),
                 sig_s=_f64(np.stack(s)), sig_c=_f64(np.stack(c)), sig_f=_f64(np.stack(f)),
                 nu=_f64([0.0, 0.0, 2.43]), watt_a=_f64([1.0, 1.0, 0.988e6]), watt_b=_f64([1.0, 1.0, 2.249e-6]))
 
 
-def _ce_pin(n_ebins, n_grid, src_energy, sigf0):
+def _ce_pin(n_ebins, n_grid, src_energy, sigf0, res_fis=None):
     h = 0.63
-    xs = ce_tables(n_grid=n_grid, sigf0=sigf0)
+    xs = ce_tables(n_grid=n_grid, sigf0=sigf0, res_fis=CE_RES_FIS if res_fis is None else res_fis)
     E = xs["energy"]
     edges = E[np.round(np.arange(n_ebins + 1) * (n_grid - 1) / n_ebins).astype(int)]
     geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((0.54,), (0, 1))], [1, 1, 1, 1, 0, 0],
@@ -245,7 +245,8 @@ def _ce_pin(n_ebins, n_grid, src_energy, sigf0):
     return geo, mats, xs
 
 
-CE_SIGF0 = 2.5   # thermal fission scale of the A=238 nuclide, tuned so k_inf < 1 (reading Q17)
+CE_RES_FIS = 0.4
+CE_SIGF0 = 8.0   # thermal fission scale of the A=238 nuclide, tuned so k_inf < 1 (reading Q17)
 
 
 def cfg3(n=1000000, n_ebins=100, seed=1, n_grid=50000, sigf0=CE_SIGF0):

@@ -1,0 +1,92 @@
+"""GPU parity: the CUDA path vs the CPU oracle, element by element, through the C ABI (-m gpu)."""
+import math
+
+import numpy as np
+import pytest
+
+from paper_2506_00263_b200 import workloads as W
+from tests.parity import assert_same, run_both
+
+pytestmark = pytest.mark.gpu
+
+SCHEMES = [("stack", "fused"), ("stack", "split"), ("async", "fused"), ("async", "split")]
+
+
+def small_cases():
+    return {
+        "cfg0": W.cfg0(),                                             # full size (1e5)
+        "cfg1": W.cfg1(n=30011, n_inactive=2, n_active=3),             # ragged
+        "cfg2": W.cfg2(n=40003, n_inactive=1, n_active=2),
+        "cfg3": W.cfg3(n=20011, n_ebins=100),
+        "cfg4": W.cfg4(n=20011, n_inactive=1, n_active=2),
+    }
+
+
+def test_device_primitives_bit_exact():
+    import torch
+    from oracle import orc
+    from paper_2506_00263_b200 import tdr
+    L = orc.lib()
+    rng = np.random.default_rng(3)
+    x = np.concatenate([rng.uniform(0, 1, 50000), np.exp(rng.uniform(-30, 30, 50000)), [2.0 ** -53, 1 - 2.0 ** -53, 1.0]])
+    got = tdr.dev_det_log(torch.from_numpy(x).cuda()).cpu().numpy()
+    ref = np.array([L.orc_det_log(float(v)) for v in x])
+    assert np.array_equal(got.view(np.uint64), ref.view(np.uint64))
+    ids = rng.integers(0, 2 ** 63, 20000).astype(np.uint64)
+    for (gen, seg, pur, j) in [(0, 1, 0, 0), (7, 123456, 3, 5), (65535, 2 ** 24, 15, 4095 * 2), (3, 0, 6, 1)]:
+        got = tdr.dev_draw(0xDEADBEEF12345, torch.from_numpy(ids.view(np.int64)).cuda(), gen, seg, pur, j).cpu().numpy()
+        ref = np.array([L.orc_draw(0xDEADBEEF12345, int(i), gen, seg, pur, j) for i in ids])
+        assert np.array_equal(got, ref)
+
+
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+def test_parity_all_configs(name, scheme, decomp):
+    p = small_cases()[name]
+    o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+    assert_same(o, g, f"{name}/{scheme}/{decomp}")
+    assert d["kernel_launches"] > 0
+
+
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+def test_small_window_forces_refill_and_secondaries(scheme, decomp):
+    """Window far below N: on-demand sourcing (make_work) refills slots; CE fixed source exercises the secondary ring."""
+    p = W.cfg3(n=5003, n_ebins=1)
+    o, g, _ = run_both(p, scheme=scheme, decomposition=decomp, window=1024)
+    assert_same(o, g, "cfg3/window=1024")
+    p = W.cfg1(n=7001, n_inactive=1, n_active=1)
+    o, g, _ = run_both(p, scheme=scheme, decomposition=decomp, window=512)
+    assert_same(o, g, "cfg1/window=512")
+
+
+@pytest.mark.parametrize("scheme", ["stack", "async"])
+def test_edge_cases(scheme):
+    for p in (W.cfg0(n=1), W.cfg0(n=31), W.cfg0(n=33), W.slab(1.3, 1.7, n=10007), W.cfg3(n=257, n_ebins=10000),
+              W.ce_slowing_down(A=16.0, n=2003)):
+        o, g, _ = run_both(p, scheme=scheme)
+        assert_same(o, g, p.name)
+    p = W.cfg2(n=3001, n_inactive=1, n_active=1)
+    p.geometry["bc"][:] = 0                                  # vacuum everywhere: leak paths
+    o, g, _ = run_both(p, scheme=scheme)
+    assert_same(o, g, "cfg2/vacuum")
+    assert g["totals"]["n_leak"] > 0
+
+
+def test_closed_forms_on_gpu_results():
+    from paper_2506_00263_b200 import tdr
+    P = tdr.Problem(W.cfg0())
+    g = P.run()
+    P.close()
+    n = 100000
+    assert abs(g["totals"]["n_coll"] / n - 1 / 0.3) < 4 * math.sqrt(0.7 / 0.09 / n)
+    assert abs(g["flux"][0] / 2 ** 24 / n - 1 / 0.3) < 4 * (1 / 0.3) / math.sqrt(n)
+
+
+def test_errors_are_reported_not_thrown():
+    from paper_2506_00263_b200 import tdr
+    P = tdr.Problem(W.cfg0())
+    with pytest.raises(tdr.TdrError):
+        P.read_tallies()                                     # TDR_ESTATE before any run
+    with pytest.raises(tdr.TdrError):
+        P.set_option("scheme", "bogus")
+    P.close()
