@@ -1,0 +1,250 @@
+#!/usr/bin/env python
+"""bench.py — particle-events/s (transport segments/s) and histories/s of the TDR transport hot path.
+
+A "step" is one pass of the whole hot path over one batch: BASELINE.json configs[1] in full
+(7-group k-eigenvalue pin cell, 1e6 particles/generation, 20 inactive + 50 active generations), i.e. one
+tdr_run_k_eigenvalue call: source, XS lookup, move, tally, collide/surface, remap, fission bank, population
+control and k update for 70 generations.  `value` is timed with the problem resident on the device; `e2e`
+goes through the C ABI from HOST buffers (tdr_init_problem uploads the tables, tdr_read_tallies downloads
+the results) inside the timed region.  Multi-GPU: independent batches per rank (different seeds), no
+collective on the data path -> "weak" scaling.  `--impl reference` times the CPU oracle.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "particle_events_per_sec"
+UNIT = "segments/s"
+WORKLOAD = "cfg1: 7-group k-eigenvalue pin cell, 1e6 particles/gen, 20 inactive + 50 active generations"
+# algorithmic bytes: fused multigroup step under whole-population residency
+BYTES_PER_SEGMENT = 150.0
+BYTES_PER_HISTORY = 96.0
+
+
+def peaks():
+    try:
+        d = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.rows, self.proc = [], None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(index)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([t.strip() for t in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        mhz, mx, reasons = [], None, set()
+        for r in self.rows:
+            try:
+                mhz.append(float(r[0])); mx = float(r[1])
+            except Exception:
+                continue
+            for name, v in zip(["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"], r[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        mhz.sort()
+        return {"sm_mhz": mhz[len(mhz) // 2] if mhz else None, "sm_max_mhz": mx, "reasons": sorted(reasons), "samples": len(mhz)}
+
+
+def input_bytes(problem):
+    import numpy as np
+    n = 0
+    for d in (problem.geometry, problem.materials, problem.xs or {}):
+        for v in d.values():
+            n += v.nbytes if isinstance(v, np.ndarray) else 8
+    return n
+
+
+def output_bytes(res):
+    import numpy as np
+    return sum(v.nbytes for v in res.values() if isinstance(v, np.ndarray)) + 12 * 8 + 16
+
+
+def run_reference(args, rank, world):
+    """The oracle, as it stands, on the host cores; each step a bounded sample of the workload."""
+    if rank != 0:
+        return
+    from oracle import orc
+    from paper_2506_00263_b200 import workloads as W
+    n, gi, ga = 50000, 2, 3
+    p = W.cfg1(n=n, n_inactive=gi, n_active=ga)
+    cores = orc.lib().orc_set_threads(0)
+    segs = hist = 0
+    for i in range(args.warmup):
+        orc.run(p)
+    t0 = time.perf_counter()
+    for i in range(args.steps):
+        r = orc.run(p)
+        segs += r["totals"]["n_seg"]; hist += int(r["gen_n"].sum())
+    dt = time.perf_counter() - t0
+    v = segs / dt
+    sample = f"cfg1 at {n} particles/gen, {gi}+{ga} generations per step ({segs // max(args.steps, 1)} segments)"
+    print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+                      "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(args.steps, 1), "higher_is_better": True, "scaling": "weak",
+                      "vs_baseline": None, "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+                      "histories_per_sec": hist / dt,
+                      "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                      "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def cpu_baseline():
+    """Oracle timed on the box's host cores on a bounded sample of the same workload (about 10-30 s)."""
+    from oracle import orc
+    from paper_2506_00263_b200 import workloads as W
+    n, gi, ga = 100000, 5, 10
+    cores = orc.lib().orc_set_threads(0)
+    t0 = time.perf_counter()
+    r = orc.run(W.cfg1(n=n, n_inactive=gi, n_active=ga))
+    dt = time.perf_counter() - t0
+    segs = r["totals"]["n_seg"]
+    return {"value": segs / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+            "sample": f"cfg1 at {n} particles/gen, {gi}+{ga} generations ({segs} segments, {dt:.1f} s)",
+            "histories_per_sec": float(r["gen_n"].sum()) / dt}
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2506_00263_b200 import tdr, workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    n, gi, ga = args.particles, args.inactive, args.active
+    prob = W.cfg1(n=n, n_inactive=gi, n_active=ga, seed=1 + rank)     # independent batch per rank
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    results = {}
+    schemes = ["stack", "async"] if args.scheme == "both" else [args.scheme]
+    for scheme in schemes:
+        P = tdr.Problem(prob, device=f"cuda:{local_rank}", scheme=scheme, decomposition=args.decomposition, time_kernels=1,
+                        **({"window": args.window} if args.window else {}))
+        for _ in range(args.warmup):
+            P.run_k_eigenvalue(n, gi, ga, prob.seed)
+        flush = torch.empty(256 << 20, dtype=torch.uint8, device=f"cuda:{local_rank}")
+        barrier()
+        sampler = ClockSampler(local_rank) if rank == 0 else None
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        segs = hist = launches = 0
+        step_ms = 0.0; step_launches = 0
+        e0.record()
+        for _ in range(args.steps):
+            flush.zero_()                                             # L2 flush between timed iterations
+            P.run_k_eigenvalue(n, gi, ga, prob.seed)
+            d = P.diagnostics()
+            launches += d["kernel_launches"]; step_ms += d["step_ms"]; step_launches += d["step_launches"]
+        e1.record()
+        barrier()
+        ms = e0.elapsed_time(e1)
+        clocks = sampler.stop() if sampler else None
+        res = P.read_tallies(history=False, bank=False)
+        seg_step, hist_step = res["totals"]["n_seg"], int(res["gen_n"].sum())      # identical every step (same seed)
+        segs, hist = seg_step * args.steps, hist_step * args.steps
+        P.close()
+        # e2e: host buffers in, host buffers out, through the C ABI
+        barrier()
+        t0 = time.perf_counter()
+        e2e_segs = 0; bi = bo = 0
+        for _ in range(args.steps):
+            Q = tdr.Problem(prob, device=f"cuda:{local_rank}", scheme=scheme, decomposition=args.decomposition,
+                            **({"window": args.window} if args.window else {}))
+            r = Q.run()
+            e2e_segs += r["totals"]["n_seg"]; bi = input_bytes(prob); bo = output_bytes(r)
+            Q.close()
+        barrier()
+        e2e_s = time.perf_counter() - t0
+        t = torch.tensor([ms, e2e_s, float(segs), float(hist), float(e2e_segs), float(launches)], dtype=torch.float64, device=f"cuda:{local_rank}")
+        if world > 1:
+            mx = t.clone(); dist.all_reduce(mx, op=dist.ReduceOp.MAX)
+            sm = t.clone(); dist.all_reduce(sm, op=dist.ReduceOp.SUM)
+            ms, e2e_s = mx[0].item(), mx[1].item()
+            segs, hist, e2e_segs, launches = sm[2].item(), sm[3].item(), sm[4].item(), sm[5].item()
+        peak, peak_src = peaks()
+        alg_bytes = BYTES_PER_SEGMENT * seg_step + BYTES_PER_HISTORY * hist_step       # one step, this rank
+        ach = (alg_bytes * args.steps / 1e9) / (step_ms / 1e3) if step_ms > 0 else 0.0
+        results[scheme] = {
+            "value": segs / (ms / 1e3), "histories_per_sec": hist / (ms / 1e3), "ms_per_step": ms / max(args.steps, 1),
+            "e2e": {"value": e2e_segs / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo},
+            "gpu_launches": int(launches), "clocks": clocks, "k_mean": res["k_mean"],
+            "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                         "peak_source": peak_src, "kernel": "k_step" if scheme == "stack" else "k_async",
+                         "kernel_share_of_step": step_ms / ms if ms > 0 else None,
+                         "avg_launch_us": 1e3 * step_ms / max(step_launches, 1),
+                         "algorithmic_bytes_per_launch": alg_bytes * args.steps / max(step_launches, 1)},
+        }
+    if rank == 0:
+        first = results[schemes[0]]
+        line = {"metric": METRIC, "value": first["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+                "ms_per_step": first["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+                "data": "synthetic", "config": {"workload": WORKLOAD if (n, gi, ga) == (1000000, 20, 50) else f"cfg1 at {n}/gen, {gi}+{ga} generations",
+                                                "scheme": schemes[0], "decomposition": args.decomposition, "particles_per_gen": n,
+                                                "generations": gi + ga, "l2": "flushed between timed steps (256 MiB write)",
+                                                "sharding": "independent batches per rank, no data-path collective"},
+                "histories_per_sec": first["histories_per_sec"], "e2e": first["e2e"], "gpu_launches": first["gpu_launches"],
+                "clocks": first["clocks"], "roofline": first["roofline"], "schemes": {k: {kk: vv for kk, vv in v.items() if kk != "clocks"} for k, v in results.items()}}
+        if world == 1 and not args.no_cpu_baseline:
+            line["cpu_baseline"] = cpu_baseline()
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="both", choices=["stack", "async", "both"])
+    ap.add_argument("--decomposition", default="fused", choices=["fused", "split"])
+    ap.add_argument("--particles", type=int, default=1000000)
+    ap.add_argument("--inactive", type=int, default=20)
+    ap.add_argument("--active", type=int, default=50)
+    ap.add_argument("--window", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1")); local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

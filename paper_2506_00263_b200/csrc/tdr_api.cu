@@ -281,7 +281,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
   u64 n0 = R.src_total < W ? R.src_total : W;
   const int first = p->split ? EV_LOOKUP : 0;
   if ((rc = source(p->stacks[first], ctr + C_STACK0 + first, 0, n0))) return rc;
-  int cur = 0;
+  int cur = 0; u64 n_in = n0;
   const int g_step = grid_for(p, k_step<CE>, smem);
   SplitGrids sg; if (p->split) split_grids<CE>(p, smem, sg);
   for (;;) {
@@ -303,7 +303,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
     CK(cudaStreamSynchronize(st));
     if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
     alive = p->split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + cur];
-    p->diag.events[1] += alive;
+    p->diag.events[1] += n_in; n_in = alive;
     h_sec_tail = h[C_SEC_TAIL];
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
     u64 head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;
@@ -315,6 +315,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
       u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;
       int slot = p->split ? EV_LOOKUP : cur;
       if ((rc = source(p->stacks[slot], ctr + C_STACK0 + slot, n_sec, n))) return rc;
+      n_in = n;
     }
   }
   return 0;
