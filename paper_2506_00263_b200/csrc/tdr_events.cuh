@@ -38,8 +38,35 @@ __device__ __forceinline__ void acc_flush(BlockAcc *a, const DevOut &o, i64 P, i
   else if (t == TDR_T_COUNT + 7) { if (a->Pc) atomicAdd(&o.PPc[1], (u64)a->Pc); }
 }
 
+// Block-private tallies in shared memory (finalize hook): used when the tally has few bins, where
+// every score would otherwise hit the same few global addresses.  An int64 bin is two 32-bit words updated with
+// native shared atomics; the carry out of the low word is added to the high word, so the sum is exact mod 2^64.
+#define PRIV_MAX_BINS 256
+struct TallyPriv { u32 *flux_lo, *flux_hi, *coll_lo, *coll_hi; int n; };
+
+__device__ __forceinline__ TallyPriv priv_init(const DevProb &P, void *mem) {
+  TallyPriv t; t.n = P.n_bins <= PRIV_MAX_BINS ? (int)P.n_bins : 0;
+  u32 *w = (u32 *)mem;
+  t.flux_lo = w; t.flux_hi = w + t.n; t.coll_lo = w + 2 * t.n; t.coll_hi = w + 3 * t.n;
+  for (int i = threadIdx.x; i < 4 * t.n; i += blockDim.x) w[i] = 0;
+  return t;
+}
+__device__ __forceinline__ void priv_add(u32 *lo, u32 *hi, u32 bin, u64 val) {
+  u32 vl = (u32)val, vh = (u32)(val >> 32);
+  u32 old = atomicAdd(&lo[bin], vl);
+  vh += (u32)(((u64)old + vl) >> 32);
+  if (vh) atomicAdd(&hi[bin], vh);
+}
+__device__ __forceinline__ void priv_flush(const TallyPriv &t, const DevOut &o) {   // after __syncthreads()
+  for (int i = threadIdx.x; i < t.n; i += blockDim.x) {
+    u64 f = ((u64)t.flux_hi[i] << 32) | t.flux_lo[i], c = ((u64)t.coll_hi[i] << 32) | t.coll_lo[i];
+    if (f) atomicAdd(&o.flux[i], f);
+    if (c) atomicAdd(&o.coll[i], c);
+  }
+}
+
 // warp-cooperative tally: every lane of the warp calls it (valid = lane has a score)
-__device__ __forceinline__ void tally_add(u64 *arr, u64 bin, i64 val, bool valid) {
+__device__ __forceinline__ void tally_add(u64 *arr, u32 *lo, u32 *hi, bool priv, u64 bin, i64 val, bool valid) {
   u32 m = __ballot_sync(FULL, valid);
   if (m == 0) return;
   int leader = __ffs(m) - 1;
@@ -47,9 +74,9 @@ __device__ __forceinline__ void tally_add(u64 *arr, u64 bin, i64 val, bool valid
   bool same = __all_sync(FULL, !valid || bin == b0);
   if (same) {
     i64 s = warp_sum_i64(valid ? val : 0);
-    if ((threadIdx.x & 31) == leader) atomicAdd(&arr[b0], (u64)s);
+    if ((threadIdx.x & 31) == leader) { if (priv) priv_add(lo, hi, (u32)b0, (u64)s); else atomicAdd(&arr[b0], (u64)s); }
   } else if (valid) {
-    atomicAdd(&arr[bin], (u64)val);
+    if (priv) priv_add(lo, hi, (u32)bin, (u64)val); else atomicAdd(&arr[bin], (u64)val);
   }
 }
 
@@ -136,7 +163,7 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
 
 // ---------------------------------------------------------------------------------- T5 TALLY (warp-cooperative)
 template <bool CE>
-__device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, const DevRun &R, const Part &p, bool valid,
+__device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, const TallyPriv &tp, const DevRun &R, const Part &p, bool valid,
                                          double d, double St, double nsf, u32 flags, i64 &accP, i64 &accPc) {
   int e = -1;
   if (valid) {
@@ -152,8 +179,8 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
   if (R.active) {
     u64 bin = 0;
     if (e >= 0) bin = ((((u64)p.mz * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;
-    tally_add(o.flux, bin, fixp(d, P.scale), e >= 0);
-    tally_add(o.coll, bin, fixp(1.0, P.scale), e >= 0 && collide);
+    tally_add(o.flux, tp.flux_lo, tp.flux_hi, tp.n > 0, bin, fixp(d, P.scale), e >= 0);
+    tally_add(o.coll, tp.coll_lo, tp.coll_hi, tp.n > 0, bin, fixp(1.0, P.scale), e >= 0 && collide);
   }
 }
 

@@ -1,7 +1,49 @@
-// tdr_split.cuh — decomposed task scheme under the stack scheme: placeholder until the kernels land.
+// tdr_split.cuh — decomposed task scheme under stack-based remapping:
+// five event types (LOOKUP, MOVE, TALLY, COLLIDE, SURFACE), one index stack and one kernel per event.
+// One remap iteration launches the five kernels in flow order, each popping its own stack (count read on
+// the device) and pushing every particle onto the stack of its next event; a kernel whose stack is empty
+// returns at once.  Dead lanes call make_work in place (COLLIDE / SURFACE) and re-enter at LOOKUP.
 #pragma once
-#include "tdr_stack.cuh"
-struct tdr_problem;
+#include "tdr_exec.cuh"
+
+struct StackSet { u32 *s[EV_COUNT]; u64 *cnt; };      // cnt[e] = device counter of stack e
+
+template <bool CE, int EV>
+__global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun R, Soa S, StackSet K, int zero_ev) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  const TallyPriv tp = stage_priv(P, smem);
+  acc_init(&acc);
+  if (blockIdx.x == 0 && threadIdx.x == 0 && zero_ev >= 0) K.cnt[zero_ev] = 0;   // the stack the previous kernel drained
+  const u64 n_in = K.cnt[EV];
+  i64 accP = 0, accPc = 0;
+  for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_in; i0 += (u64)gridDim.x * blockDim.x) {
+    u64 i = i0 + threadIdx.x;
+    bool valid = i < n_in;
+    u32 slot = valid ? K.s[EV][i] : 0;
+    Part p; int nch, csrc;
+    int next = exec_event<CE, EV>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, EV_LOOKUP);
+    if (EV == EV_COLLIDE || EV == EV_SURFACE) {
+      if (EV == EV_COLLIDE) push_children(O, R, &acc, p, nch, csrc);
+      bool dead = valid && next == NEXT_DEAD;
+      if (make_work<CE>(P, mg, R, &acc, p, dead)) { store_part<CE>(S, slot, p); next = EV_LOOKUP; }
+      stack_push(K.s[EV_LOOKUP], &K.cnt[EV_LOOKUP], slot, next == EV_LOOKUP);
+    } else if (EV == EV_TALLY) {
+      stack_push(K.s[EV_COLLIDE], &K.cnt[EV_COLLIDE], slot, next == EV_COLLIDE);
+      stack_push(K.s[EV_SURFACE], &K.cnt[EV_SURFACE], slot, next == EV_SURFACE);
+    } else {
+      const int nx = EV == EV_LOOKUP ? EV_MOVE : EV_TALLY;
+      stack_push(K.s[nx], &K.cnt[nx], slot, next == nx);
+    }
+  }
+  acc_flush(&acc, O, accP, accPc);
+  if (EV == EV_TALLY) priv_flush(tp, O);
+}
+
 struct SplitGrids { int g[EV_COUNT]; };
-template <bool CE> static void split_grids(tdr_problem *, size_t, SplitGrids &) {}
-template <bool CE> static int split_iteration(tdr_problem *, DevRun &, size_t, const SplitGrids &) { return TDR_EINVAL; }
+
+// host side -----------------------------------------------------------------------------------------------
+struct tdr_problem;
+template <bool CE> static void split_grids(tdr_problem *p, size_t smem, SplitGrids &sg);
+template <bool CE> static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg);

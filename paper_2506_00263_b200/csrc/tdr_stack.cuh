@@ -84,6 +84,8 @@ __device__ __forceinline__ const double *stage_mg(const DevProb &P, double *smem
   for (int i = threadIdx.x; i < P.mg_doubles; i += blockDim.x) smem[i] = P.mg[i];
   return smem;
 }
+// dynamic shared memory = [MG table | private tally words]; host side: smem_bytes()
+__device__ __forceinline__ TallyPriv stage_priv(const DevProb &P, double *smem) { return priv_init(P, smem + P.mg_doubles); }
 
 // ---------------------------------------------------------------------------------- A1 SOURCE: fill slots [0, n)
 template <bool CE>
@@ -115,6 +117,7 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
+  const TallyPriv tp = stage_priv(P, smem);
   acc_init(&acc);
   const u64 n_in = *count_in;
   i64 accP = 0, accPc = 0;
@@ -129,7 +132,7 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
       ev_lookup<CE>(P, mg, p, St, nsf, gi, f);
       ev_move(P, R.seed, R.gen, p, St, d, flags);
     }
-    ev_tally<CE>(P, O, R, p, valid && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
+    ev_tally<CE>(P, O, tp, R, p, valid && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
     bool alive = false; int nch = 0, csrc = 0;
     if (valid) {
       if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
@@ -142,6 +145,7 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
     stack_push(stack_out, count_out, slot, alive);
   }
   acc_flush(&acc, O, accP, accPc);
+  priv_flush(tp, O);
 }
 
 // ---------------------------------------------------------------------------------- A9 population control (D2)
