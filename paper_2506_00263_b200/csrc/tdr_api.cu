@@ -31,6 +31,8 @@ struct tdr_problem {
   int blocks_per_sm = 0;                   // 0 = occupancy query
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
+  int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
+  int sync_every = 8;                      // stack scheme: remap iterations launched per counter read-back
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
   // carved pointers (valid during/after a run)
@@ -162,10 +164,11 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   if (k == "scheme") { if (v == "stack") p->scheme = 0; else if (v == "async") p->scheme = 1; else return fail(TDR_EINVAL, "scheme must be stack|async"); }
   else if (k == "decomposition") { if (v == "fused") p->split = 0; else if (v == "split") p->split = 1; else return fail(TDR_EINVAL, "decomposition must be fused|split"); }
   else if (k == "window") { long long w = atoll(value); if (w < 32) return fail(TDR_EINVAL, "window too small"); p->window = (u64)w; }
-  else if (k == "stash_links") { int n = atoi(value); if (n < 4 || n > 64) return fail(TDR_EINVAL, "stash_links in [4,64]"); p->stash_links = n; }
+  else if (k == "stash_links") { int n = atoi(value); if (n < 8 || n > 64) return fail(TDR_EINVAL, "stash_links in [8,64]"); p->stash_links = n; }
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
+  else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
 }
@@ -199,11 +202,11 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   DevOut o;
   o.flux = c.take<u64>(p->dp.n_bins); o.coll = c.take<u64>(p->dp.n_bins); o.leak = c.take<u64>(6);
   o.totals = c.take<u64>(TDR_T_COUNT); o.PPc = c.take<u64>(2); o.err = c.take<int>(1);
-  u64 bank_cap = 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + 4096;
+  u64 bank_cap = 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + (1ull << 20);
   tdr_site *bank = c.take<tdr_site>(bank_cap), *src = c.take<tdr_site>(src_cap), *sec = c.take<tdr_site>(sec_cap);
   u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
   u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
-  AsyncMem am; async_layout(c, W, p->num_sms, am);
+  AsyncMem am; async_layout(c, W, sec_cap, am);
   if (assign) {
     p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
     p->bank = bank; p->srcbank = src; p->sec = sec; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
@@ -258,12 +261,44 @@ static int check_dev_err(tdr_problem *p, int code) {
 
 #define LAUNCH_CHECK() CK(cudaGetLastError())
 
+// ---------------------------------------------------------------------------------- split decomposition (stack scheme)
+template <bool CE>
+static void split_grids(tdr_problem *p, size_t smem, SplitGrids &sg) {
+  sg.g[EV_LOOKUP] = grid_for(p, k_event<CE, EV_LOOKUP>, smem);
+  sg.g[EV_MOVE] = grid_for(p, k_event<CE, EV_MOVE>, smem);
+  sg.g[EV_TALLY] = grid_for(p, k_event<CE, EV_TALLY>, smem);
+  sg.g[EV_COLLIDE] = grid_for(p, k_event<CE, EV_COLLIDE>, smem);
+  sg.g[EV_SURFACE] = grid_for(p, k_event<CE, EV_SURFACE>, smem);
+}
+
+// one remap iteration: one kernel per event stack, in flow order; an empty stack costs an empty launch
+template <bool CE>
+static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg, int cap_blocks) {
+  cudaStream_t st = p->stream;
+  StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
+  K.cnt = p->ctr + C_STACK0;
+  auto g = [&](int e) { return sg.g[e] < cap_blocks ? sg.g[e] : cap_blocks; };
+  KTimer t(p, true);
+  k_event<CE, EV_LOOKUP><<<g(EV_LOOKUP), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_SURFACE);
+  k_event<CE, EV_MOVE><<<g(EV_MOVE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_LOOKUP);
+  k_event<CE, EV_TALLY><<<g(EV_TALLY), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_MOVE);
+  k_event<CE, EV_COLLIDE><<<g(EV_COLLIDE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_TALLY);
+  k_event<CE, EV_SURFACE><<<g(EV_SURFACE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_COLLIDE);
+  LAUNCH_CHECK(); p->diag.kernel_launches += 5;
+  return 0;
+}
+
 // ---------------------------------------------------------------------------------- stack scheme, one generation
+static size_t smem_bytes(const tdr_problem *p) {      // dynamic shared memory = [MG table | private tally words]
+  size_t priv = p->dp.n_bins <= PRIV_MAX_BINS ? (size_t)p->dp.n_bins * 16 : 0;
+  return (size_t)p->dp.mg_doubles * sizeof(double) + priv;
+}
+
 template <bool CE>
 static int run_stack(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
-  const size_t smem = (size_t)p->dp.mg_doubles * sizeof(double);
-  u64 *ctr = p->ctr; u64 *h = p->h_ctr, *hup = p->h_ctr + 32;
+  const size_t smem = smem_bytes(p);
+  u64 *ctr = p->ctr; u64 *h = p->h_ctr;
   const int g_src = grid_for(p, k_source<CE>, smem);
   const u64 W = p->W;
   u64 h_src_next = 0, h_sec_tail = 0, h_sec_head = 0;
@@ -271,53 +306,87 @@ static int run_stack(tdr_problem *p, DevRun R) {
     k_source<CE><<<g_src, 256, smem, st>>>(p->dp, p->out, R, p->soa, stack, count, h_sec_head, n_sec, h_src_next, n);
     LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.events[0] += n;
     h_sec_head += n_sec; h_src_next += n - n_sec;
-    hup[0] = h_src_next; hup[1] = h_sec_head;
-    CK(cudaMemcpyAsync(ctr + C_SRC_NEXT, hup, 8, cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, hup + 1, 8, cudaMemcpyHostToDevice, st));
-    CK(cudaStreamSynchronize(st));                 // hup is reused
     return 0;
   };
   int rc;
   u64 n0 = R.src_total < W ? R.src_total : W;
-  const int first = p->split ? EV_LOOKUP : 0;
-  if ((rc = source(p->stacks[first], ctr + C_STACK0 + first, 0, n0))) return rc;
-  int cur = 0; u64 n_in = n0;
-  const int g_step = grid_for(p, k_step<CE>, smem);
+  // fused: two index stacks, three rotating counters (in, out, the one to clear); split: one stack per event
+  u64 it = 0;
+  if (!p->split) { if ((rc = source(p->stacks[0], ctr + C_STACK0, 0, n0))) return rc; }
+  else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, 0, n0))) return rc;
+  u64 n_in = n0;
+  const int g_step = p->split ? 0 : grid_for(p, k_step<CE>, smem);
   SplitGrids sg; if (p->split) split_grids<CE>(p, smem, sg);
   for (;;) {
     R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
-    u64 alive;
-    if (!p->split) {
-      CK(cudaMemsetAsync(ctr + C_STACK0 + (1 - cur), 0, 8, st));
-      {
+    // the out count never exceeds the in count (dead lanes are reborn in place), so n_in bounds every launch of
+    // this batch: launch `batch` remap iterations back to back and read the counters once
+    const int batch = n_in * 4 > W ? 1 : p->sync_every;
+    u64 blocks64 = (n_in + 255) / 256; int cap_blocks = blocks64 > (1u << 30) ? (1 << 30) : (int)blocks64;
+    if (cap_blocks < 1) cap_blocks = 1;
+    for (int b = 0; b < batch; b++) {
+      if (!p->split) {
+        const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
         KTimer t(p, true);
-        k_step<CE><<<g_step, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[cur], ctr + C_STACK0 + cur, p->stacks[1 - cur], ctr + C_STACK0 + 1 - cur);
-      }
-      LAUNCH_CHECK(); p->diag.kernel_launches++;
-      cur = 1 - cur;
-    } else {
-      if ((rc = split_iteration<CE>(p, R, smem, sg))) return rc;
+        k_step<CE><<<g_step < cap_blocks ? g_step : cap_blocks, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+                                                                               p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr);
+        LAUNCH_CHECK(); p->diag.kernel_launches++;
+      } else if ((rc = split_iteration<CE>(p, R, smem, sg, cap_blocks))) return rc;
+      it++; p->diag.iterations++;
     }
-    p->diag.iterations++;
     CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
-    alive = p->split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + cur];
-    p->diag.events[1] += n_in; n_in = alive;
+    const u64 alive = p->split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + it % 3];
+    n_in = alive;
     h_sec_tail = h[C_SEC_TAIL];
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
-    u64 head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;
-    if (head != h[C_SEC_HEAD]) { hup[1] = head; CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, hup + 1, 8, cudaMemcpyHostToDevice, st)); CK(cudaStreamSynchronize(st)); }
-    h_sec_head = head;
+    h_sec_head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;          // claims past the limit got nothing
+    const u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
     if (alive == 0) {
-      u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
       if (pend + rem == 0) break;
       u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;
-      int slot = p->split ? EV_LOOKUP : cur;
-      if ((rc = source(p->stacks[slot], ctr + C_STACK0 + slot, n_sec, n))) return rc;
+      R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
+      if (!p->split) { if ((rc = source(p->stacks[it & 1], ctr + C_STACK0 + it % 3, n_sec, n))) return rc; }
+      else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, n_sec, n))) return rc;
       n_in = n;
+    } else if (h[C_SEC_HEAD] != h_sec_head) {
+      h[33] = h_sec_head;                                   // clamp the overshoot of the claim cursor (the limit grows later)
+      CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, h + 33, 8, cudaMemcpyHostToDevice, st));
+      CK(cudaStreamSynchronize(st));
     }
   }
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------- asynchronous scheme, one generation
+template <bool CE, bool SPLIT>
+static int launch_async(tdr_problem *p, const DevRun &R, size_t smem) {
+  int grid = grid_for(p, k_async<CE, SPLIT>, smem);
+  KTimer t(p, true);
+  k_async<CE, SPLIT><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull);
+  return 0;
+}
+
+template <bool CE>
+static int run_async(tdr_problem *p, DevRun R) {
+  cudaStream_t st = p->stream;
+  const size_t smem = smem_bytes(p) + 8 * (size_t)STASH_WORDS(p->stash_links) * 4;
+  R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
+  if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
+  k_async_init<<<1, 64, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
+  LAUNCH_CHECK();
+  if (p->split) launch_async<CE, true>(p, R, smem); else launch_async<CE, false>(p, R, smem);
+  LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
+  u64 *h = p->h_ctr;
+  CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(h + 40, p->am.actr, AC_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  p->diag.spills += h[40 + AC_SPILLS]; p->diag.fetches += h[40 + AC_FETCHES]; p->diag.make_work_calls += h[40 + AC_MAKEWORK];
+  p->diag.events[1] += h[40 + AC_EVENTS]; p->diag.events[0] += R.src_total;
+  int rc;
+  if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
+  if (h[C_PENDING] != 0) return fail(TDR_ESTATE, "asynchronous scheme left %llu particles outstanding", h[C_PENDING]);
   return 0;
 }
 

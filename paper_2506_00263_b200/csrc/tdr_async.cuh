@@ -1,16 +1,20 @@
 // tdr_async.cuh — asynchronous remapping (section 3.2): ONE persistent kernel per generation.
 //  * work link: a warp-sized array of particle slots that all wait for the same event, with the
 //    event id, the fill count and a next pointer.  Particle state stays in the SoA arrays (DESIGN.md reading
-//    Q21); links carry 4-byte slot indices.  Free slots travel the same way, as links of event EV_FREE.
+//    Q21); links carry 4-byte slot indices.
 //  * stash: per warp, in shared memory: L links, a free list, a full list and a table
 //    event id -> partially filled link.  Inserting fills the partial link of that event; a link that fills up
 //    moves to the full list; a processed link returns to the free list.
-//  * spill / fetch: global links come from one arena; three sets of AQ queues (empty links,
-//    work links, free-slot links), each queue one 64-bit word (head << 32 | tail).  A warp claims a queue by
-//    atomicExch with the null queue, edits the list privately, and swaps it back; nobody ever waits on an owner.
-//  * make_work: called by a warp with no full link; claims source indices with one atomicAdd.
-//  * load balance / termination: a global count of starved warps makes busy warps spill; a global count of live
-//    particles tells a starved warp when to exit.  No grid-wide synchronisation anywhere.
+//  * spill / fetch: global links come from one arena; two sets of AQ queues (empty links,
+//    work links), each queue one 64-bit word (head << 32 | tail).  A warp claims a queue by atomicExch with the
+//    null queue, edits the list privately, and swaps it back; nobody ever waits on an owner.
+//  * make_work: a lane whose particle died claims the next source index (or a pending secondary)
+//    and is reborn in the same slot; a warp with no runnable link claims up to 32 fresh slots and fills them.
+//  * load balance / termination: a global count of starved warps makes busy warps spill; a global count of
+//    outstanding particles (source not yet dead + secondaries) tells a starved warp when to exit.  The count is
+//    flushed lazily (when a warp goes idle), so a stale zero can only make an idle warp leave early; a warp that
+//    holds work never leaves, and every warp re-checks the source, the secondary ring and the global queues
+//    before it leaves, so no work is stranded.  No grid-wide synchronisation anywhere.
 #pragma once
 #include "tdr_exec.cuh"
 
@@ -19,20 +23,22 @@
 #define NOLINK 0xFFFFFFFFu
 #define NOSLOT 0xFFFFFFFFu
 
+
 struct GLink { u32 idx[32]; u32 count, ev, next, pad; };
-enum { AC_GWORK = 0, AC_GFREE, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_COUNT = 8 };
-struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work, *q_free; u64 *actr; };
+enum { AC_GWORK = 0, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_EVENTS, AC_COUNT = 8 };
+struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *actr; u64 *sec_flag; };
 
 template <class C>
-static void async_layout(C &c, u64 W, int num_sms, AsyncMem &am) {
+static void async_layout(C &c, u64 W, u64 sec_cap, AsyncMem &am) {
   am.n_links = 2 * (W / 32) + 4096;
   am.links = c.template take<GLink>(am.n_links);
-  am.q_empty = c.template take<u64>(AQ); am.q_work = c.template take<u64>(AQ); am.q_free = c.template take<u64>(AQ);
+  am.q_empty = c.template take<u64>(AQ); am.q_work = c.template take<u64>(AQ);
   am.actr = c.template take<u64>(AC_COUNT);
-  (void)num_sms;
+  am.sec_flag = c.template take<u64>(sec_cap);
 }
 
 __device__ __forceinline__ u64 ld_vol(const u64 *p) { return *(const volatile u64 *)p; }
+__device__ __forceinline__ u64 global_ns() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 
 // ---------------------------------------------------------------------------------- global queues (lane 0 only)
 __device__ __forceinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine) {
@@ -66,22 +72,23 @@ __device__ __forceinline__ u32 q_pop(GLink *links, u64 *qs, u32 start) {
   return NOLINK;
 }
 
-// builds the empty-link queues: arena link i belongs to queue i % AQ
-__global__ void k_async_init(AsyncMem A) {
+// builds the empty-link queues (arena link i belongs to queue i % AQ) and resets the scheduler counters
+__global__ void k_async_init(AsyncMem A, u64 *outstanding, u64 n_source, u64 *slot_next, u64 *starved) {
   u32 q = threadIdx.x;
   if (q < AQ) {
     u32 last = NOLINK, first = NOLINK;
     for (u64 i = q; i < A.n_links; i += AQ) { if (first == NOLINK) first = (u32)i; A.links[i].next = (i + AQ < A.n_links) ? (u32)(i + AQ) : NOLINK; last = (u32)i; }
     A.q_empty[q] = first == NOLINK ? NULLQ : (((u64)first << 32) | last);
-    A.q_work[q] = NULLQ; A.q_free[q] = NULLQ;
+    A.q_work[q] = NULLQ;
   }
   if (q < AC_COUNT) A.actr[q] = 0;
+  if (q == 0) { *outstanding = n_source; *slot_next = 0; *starved = 0; }
 }
 
 // ---------------------------------------------------------------------------------- stash (per warp, shared memory)
 struct Stash {
   u32 *idx;            // [L][32]
-  int *meta;           // [0] nfree [1] nfull [2..2+EV_COUNT) partial[ev] ; then cnt[L], ev[L], freel[L], full[L]
+  int *meta;           // [0] nfree [1] nrun [2..2+EV_COUNT) partial[ev] ; then cnt[L], ev[L], freel[L], run[L]
   int L;
   __device__ __forceinline__ int &nfree() const { return meta[0]; }
   __device__ __forceinline__ int &nfull() const { return meta[1]; }
@@ -95,7 +102,6 @@ struct Stash {
 
 struct WarpCtx {                       // warp-uniform scheduler state
   Stash s; AsyncMem A; int *err; u32 lane, gw;
-  int n_free_slots;                    // free slots held in this stash
 };
 
 __device__ __forceinline__ void stash_init(const Stash &s, u32 lane) {
@@ -107,7 +113,7 @@ __device__ __forceinline__ void stash_init(const Stash &s, u32 lane) {
   __syncwarp();
 }
 
-// move stash link l (full list position fi, or fi < 0 for a partial link) to the global queues
+// spill: move stash link l (run-list position fi, or fi < 0 for a partial link) to a global link
 __device__ __forceinline__ void spill_link(WarpCtx &w, int l, int fi) {
   const Stash &s = w.s;
   int c = s.cnt(l), e = s.ev(l);
@@ -120,34 +126,53 @@ __device__ __forceinline__ void spill_link(WarpCtx &w, int l, int fi) {
   __threadfence();
   __syncwarp();
   if (w.lane == 0) {
-    q_deposit(w.A.links, e == EV_FREE ? w.A.q_free : w.A.q_work, w.gw % AQ, ((u64)g << 32) | g);
-    atomicAdd(&w.A.actr[e == EV_FREE ? AC_GFREE : AC_GWORK], 1ull); atomicAdd(&w.A.actr[AC_SPILLS], 1ull);
+    q_deposit(w.A.links, w.A.q_work, w.gw % AQ, ((u64)g << 32) | g);
+    atomicAdd(&w.A.actr[AC_GWORK], 1ull); atomicAdd(&w.A.actr[AC_SPILLS], 1ull);
     if (fi >= 0) { s.full(fi) = s.full(s.nfull() - 1); s.nfull() -= 1; } else s.partial(e) = -1;
     s.cnt(l) = 0; s.freel(s.nfree()) = l; s.nfree() += 1;
   }
-  if (e == EV_FREE) w.n_free_slots -= c;
   __syncwarp();
 }
 
-// make sure the free list has a link; spills a full link if it must ("production exceeds stash capacity")
+// fetch: bring one global work link into the stash's run list
+__device__ __forceinline__ bool fetch_link(WarpCtx &w) {
+  const Stash &s = w.s;
+  if (s.nfree() == 0) return false;
+  u32 g = NOLINK;
+  if (w.lane == 0 && ld_vol(&w.A.actr[AC_GWORK]) > 0) g = q_pop(w.A.links, w.A.q_work, w.gw);
+  g = __shfl_sync(FULL, g, 0);
+  if (g == NOLINK) return false;
+  const int c = (int)*(volatile u32 *)&w.A.links[g].count, e = (int)*(volatile u32 *)&w.A.links[g].ev;
+  const int l = s.freel(s.nfree() - 1);
+  if ((int)w.lane < c) s.idx[l * 32 + w.lane] = *(volatile u32 *)&w.A.links[g].idx[w.lane];
+  __syncwarp();
+  if (w.lane == 0) {
+    s.nfree() -= 1; s.cnt(l) = c; s.ev(l) = e; s.full(s.nfull()) = l; s.nfull() += 1;
+    atomicAdd(&w.A.actr[AC_GWORK], ~0ull); atomicAdd(&w.A.actr[AC_FETCHES], 1ull);
+    *(volatile u32 *)&w.A.links[g].next = NOLINK;
+    __threadfence();
+    q_deposit(w.A.links, w.A.q_empty, w.gw % AQ, ((u64)g << 32) | g);
+  }
+  __syncwarp();
+  return true;
+}
+
+// make sure the free list has a link; spills a runnable link if it must ("production exceeds stash capacity")
 __device__ __forceinline__ void ensure_free_link(WarpCtx &w) {
   const Stash &s = w.s;
   if (s.nfree() > 0) return;
-  int fi = -1;
-  for (int i = 0; i < s.nfull(); i++) if (s.ev(s.full(i)) == EV_FREE) fi = i;     // prefer shedding free slots
-  if (fi < 0) fi = s.nfull() - 1;
+  int fi = s.nfull() - 1;
   if (fi >= 0) spill_link(w, s.full(fi), fi);
-  else if (w.lane == 0) atomicExch(w.err, TDR_ECAPACITY);
+  else if (w.lane == 0) atomicExch(w.err, TDR_ECAPACITY);        // cannot happen while L > EV_COUNT
 }
 
-// warp-collective insert of one slot per flagged lane into the partial link of event e
+// warp-collective insert of one slot per flagged lane into the partial link of event e (PAPER.md:85)
 __device__ __forceinline__ void stash_insert(WarpCtx &w, int e, u32 value, bool pred) {
   const Stash &s = w.s;
   u32 m = __ballot_sync(FULL, pred);
   int n = __popc(m);
   if (n == 0) return;
   int rank = __popc(m & lanemask_lt()), served = 0;
-  if (e == EV_FREE) w.n_free_slots += n;
   while (served < n) {
     int pl = s.partial(e);
     if (pl < 0) {
@@ -167,4 +192,172 @@ __device__ __forceinline__ void stash_insert(WarpCtx &w, int e, u32 value, bool 
     __syncwarp();
     served += take;
   }
+}
+
+// ---------------------------------------------------------------------------------- make_work
+// Lanes flagged `want` hold a slot with no particle.  Pending secondaries first (fixed source; a record is
+// claimable once its ready flag carries its own ticket), then the primary source.  Returns true if reborn.
+template <bool CE>
+__device__ __forceinline__ bool make_work_async(const DevProb &P, const double *mg, const DevRun &R, const AsyncMem &A, BlockAcc *acc,
+                                                int *err, Part &p, bool want) {
+  const u32 lane = threadIdx.x & 31;
+  bool reborn = false;
+  u32 m = __ballot_sync(FULL, want);
+  if (m == 0) return false;
+  const int leader = __ffs(m) - 1;
+  if (!R.kmode) {
+    u64 h = 0; u32 got = 0;
+    if (lane == (u32)leader) {
+      const u32 n = (u32)__popc(m);
+      for (;;) {
+        u64 head = ld_vol(R.sec_head), tail = ld_vol(R.sec_tail);
+        if (head >= tail) break;
+        u64 take = tail - head < n ? tail - head : n;
+        if (atomicCAS(R.sec_head, head, head + take) == head) { h = head; got = (u32)take; break; }
+      }
+    }
+    h = __shfl_sync(FULL, h, leader); got = __shfl_sync(FULL, got, leader);
+    const u32 rank = (u32)__popc(m & lanemask_lt());
+    if (want && rank < got) {
+      const u64 idx = h + rank, k = idx % R.sec_cap;
+      bool ok = true;                                              // its writer is between the ticket and the flag
+      while (ld_vol(&A.sec_flag[k]) != idx + 1) { if (*(volatile int *)err) { ok = false; break; } __nanosleep(20); }
+      if (ok) { __threadfence(); tdr_site s = R.sec[k]; birth_site<CE>(P, mg, R, acc, p, s); reborn = true; }
+    }
+    m = __ballot_sync(FULL, want && !reborn);
+    if (m == 0) return reborn;
+  }
+  const int leader2 = __ffs(m) - 1;
+  u64 h = ~0ull;
+  if (lane == (u32)leader2 && ld_vol(R.src_next) < R.src_total) h = atomicAdd(R.src_next, (u64)__popc(m));
+  h = __shfl_sync(FULL, h, leader2);
+  if (want && !reborn && h != ~0ull) {
+    u64 idx = h + __popc(m & lanemask_lt());
+    if (idx < R.src_total) {
+      if (R.src_sites) { tdr_site s = R.sites[idx]; birth_site<CE>(P, mg, R, acc, p, s); }
+      else birth_primary<CE>(P, mg, R, acc, p, idx);
+      reborn = true;
+    }
+  }
+  return reborn;
+}
+
+__device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp-uniform
+  bool yes = false;
+  if ((threadIdx.x & 31) == 0) {
+    yes = ld_vol(R.src_next) < R.src_total;
+    if (!yes && !R.kmode) yes = ld_vol(R.sec_head) < ld_vol(R.sec_tail);
+  }
+  return __shfl_sync(FULL, (int)yes, 0) != 0;
+}
+
+// ---------------------------------------------------------------------------------- the persistent kernel
+template <bool CE, bool SPLIT>
+__global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  const TallyPriv tp = stage_priv(P, smem);
+  acc_init(&acc);
+  WarpCtx w;
+  w.lane = threadIdx.x & 31; w.gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w.A = A; w.err = O.err;
+  u32 *stash_mem = (u32 *)(smem + P.mg_doubles) + 4 * tp.n + (threadIdx.x >> 5) * STASH_WORDS(L);
+  w.s.idx = stash_mem; w.s.meta = (int *)(stash_mem + 32 * L); w.s.L = L;
+  stash_init(w.s, w.lane);
+  const Stash &s = w.s;
+  const int first_ev = SPLIT ? EV_LOOKUP : EV_STEP;
+  i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
+  u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
+  bool starved = false;
+  u32 n_events = 0, n_makework = 0, n_iter = 0;
+  u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
+  for (;;) {
+    int l = -1, fi = -1;
+    if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
+    else {
+      if (source_has_work(R)) {
+        // starved warp: every lane brings a slot (its own spare one, else a fresh one from the window) and claims work
+        u32 need = __ballot_sync(FULL, myfree == NOSLOT);
+        if (need) {
+          const int ld = __ffs(need) - 1; u64 b = ~0ull;
+          if (w.lane == (u32)ld && ld_vol(R.slot_next) < R.W) b = atomicAdd(R.slot_next, (u64)__popc(need));
+          b = __shfl_sync(FULL, b, ld);
+          if (b != ~0ull && myfree == NOSLOT) { u64 k = b + __popc(need & lanemask_lt()); if (k < R.W) myfree = (u32)k; }
+        }
+        Part p;
+        bool born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, myfree != NOSLOT);
+        u32 slot = myfree;
+        if (born) { store_part<CE>(S, slot, p); myfree = NOSLOT; }
+        n_makework++;
+        if (__any_sync(FULL, born)) { stash_insert(w, first_ev, slot, born); if (s.nfull() > 0) continue; }
+      }
+      int bc = 0;
+      for (int e = 0; e < EV_COUNT; e++) { int pl = s.partial(e); if (pl >= 0 && s.cnt(pl) > bc) { l = pl; bc = s.cnt(pl); } }
+      if (l < 0) {
+        if (fetch_link(w)) continue;
+        // nothing anywhere in reach: publish what this warp knows, then leave or wait (no other warp is waited for)
+        if (delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+        u64 out = 0; int er = 0;
+        if (w.lane == 0) {
+          out = ld_vol(R.outstanding); er = *(volatile int *)O.err;
+          if (out != last_out) { last_out = out; t_idle = global_ns(); }          // someone made progress
+          else if (starved && global_ns() - t_idle > deadline_ns) { atomicExch(O.err, TDR_ELOST); er = 1; }
+        }
+        out = __shfl_sync(FULL, out, 0); er = __shfl_sync(FULL, er, 0);
+        if (out == 0 || er != 0) break;
+        if (!starved) { starved = true; if (w.lane == 0) { atomicAdd(R.starved, 1ull); t_idle = global_ns(); } }
+        __nanosleep(500);
+        continue;
+      }
+    }
+    if (starved) { starved = false; if (w.lane == 0) atomicAdd(R.starved, ~0ull); }
+    // take the link out of the stash, then run its event on all lanes
+    const int c = s.cnt(l), e = s.ev(l);
+    const bool valid = (int)w.lane < c;
+    const u32 slot = valid ? s.idx[l * 32 + w.lane] : 0;
+    __syncwarp();
+    if (w.lane == 0) {
+      if (fi >= 0) { s.full(fi) = s.full(s.nfull() - 1); s.nfull() -= 1; } else s.partial(e) = -1;
+      s.cnt(l) = 0; s.freel(s.nfree()) = l; s.nfree() += 1;
+    }
+    __syncwarp();
+    Part p; int nch = 0, csrc = 0, next = NEXT_DEAD;
+    n_events += (u32)c;
+    if (!SPLIT) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
+    else switch (e) {
+      case EV_LOOKUP: next = exec_event<CE, EV_LOOKUP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
+      case EV_MOVE: next = exec_event<CE, EV_MOVE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
+      case EV_TALLY: next = exec_event<CE, EV_TALLY>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
+      case EV_COLLIDE: next = exec_event<CE, EV_COLLIDE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
+      default: next = exec_event<CE, EV_SURFACE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
+    }
+    const bool died = valid && next == NEXT_DEAD;
+    const u32 dm = __ballot_sync(FULL, died);
+    if (dm) {                                                   // only STEP / COLLIDE / SURFACE (or a lost particle) get here
+      const u32 nc = __reduce_add_sync(FULL, (u32)nch);
+      if (nc) push_children(O, R, &acc, p, nch, csrc);
+      delta += (i64)nc - (i64)__popc(dm);
+      if (make_work_async<CE>(P, mg, R, A, &acc, O.err, p, died)) { store_part<CE>(S, slot, p); next = first_ev; }
+      else if (died && myfree == NOSLOT) myfree = slot;
+    }
+    if (!SPLIT) stash_insert(w, EV_STEP, slot, next == EV_STEP);
+    else {
+      if (e == EV_LOOKUP) stash_insert(w, EV_MOVE, slot, next == EV_MOVE);
+      else if (e == EV_MOVE) stash_insert(w, EV_TALLY, slot, next == EV_TALLY);
+      else if (e == EV_TALLY) { stash_insert(w, EV_COLLIDE, slot, next == EV_COLLIDE); stash_insert(w, EV_SURFACE, slot, next == EV_SURFACE); }
+      else stash_insert(w, EV_LOOKUP, slot, next == EV_LOOKUP);
+    }
+    if ((++n_iter & 63u) == 0 && delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+    // load balance: a warp is starved and this one holds more than one runnable link -> hand one over
+    if (s.nfull() >= 2) {
+      u64 st = 0;
+      if (w.lane == 0) st = ld_vol(R.starved);
+      st = __shfl_sync(FULL, st, 0);
+      if (st > 0) spill_link(w, s.full(0), 0);
+    }
+  }
+  if (w.lane == 0) { atomicAdd(&A.actr[AC_EVENTS], (u64)n_events); atomicAdd(&A.actr[AC_MAKEWORK], (u64)n_makework); }
+  __syncthreads();
+  acc_flush(&acc, O, accP, accPc);
+  priv_flush(tp, O);
 }

@@ -58,6 +58,9 @@ struct DevRun {
                                                   // records [sec_head0, sec_limit) are complete and claimable
   tdr_site *bank; u64 bank_cap; u64 *bank_count;                        // k-mode fission bank
   u64 *hist_id; u32 *hist_nseg, *hist_ncoll; u64 *hist_count; u64 hist_cap;
+  // asynchronous scheme only: ready flags of the secondary ring (flag[t % cap] == t + 1 once record t is complete),
+  // outstanding-particle count, bump allocator of window slots, count of starved warps, window size
+  u64 *sec_flag, *outstanding, *slot_next, *starved; u64 W;
 };
 
 struct Part {

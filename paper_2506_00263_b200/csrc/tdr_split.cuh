@@ -46,4 +46,4 @@ struct SplitGrids { int g[EV_COUNT]; };
 // host side -----------------------------------------------------------------------------------------------
 struct tdr_problem;
 template <bool CE> static void split_grids(tdr_problem *p, size_t smem, SplitGrids &sg);
-template <bool CE> static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg);
+template <bool CE> static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg, int cap_blocks);

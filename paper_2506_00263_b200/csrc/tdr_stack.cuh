@@ -12,6 +12,10 @@ enum { C_SRC_NEXT = 0, C_SEC_TAIL, C_SEC_HEAD, C_BANK, C_HIST, C_NEXT_BANK, C_PE
 // event ids (split decomposition; async scheme)
 enum { EV_LOOKUP = 0, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_STEP, EV_FREE, EV_COUNT };
 
+// asynchronous scheme: a claimed secondary may still be read this many records behind the tail, so the ring keeps
+// this much headroom (>= the number of resident threads, 148 x 2048)
+#define SEC_MARGIN (1ull << 19)
+
 __device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
 // warp-collective push of one index per flagged lane
@@ -41,7 +45,13 @@ __device__ __forceinline__ void push_children(const DevOut &O, const DevRun &R, 
     u64 t = base + excl + c;
     tdr_site s = make_site(R, p, src, (u32)c);
     if (R.kmode) { if (t < R.bank_cap) R.bank[t] = s; else atomicExch(O.err, TDR_ECAPACITY); }
-    else { if (t - R.sec_head0 < R.sec_cap) R.sec[t % R.sec_cap] = s; else atomicExch(O.err, TDR_ECAPACITY); }
+    else if (!R.sec_flag) { if (t - R.sec_head0 < R.sec_cap) R.sec[t % R.sec_cap] = s; else atomicExch(O.err, TDR_ECAPACITY); }
+    else {                                                       // asynchronous scheme: publish with a ready flag
+      const u64 k = t % R.sec_cap;
+      if (t - *(const volatile u64 *)R.sec_head < R.sec_cap - SEC_MARGIN) {
+        R.sec[k] = s; __threadfence(); *(volatile u64 *)&R.sec_flag[k] = t + 1;
+      } else atomicExch(O.err, TDR_ECAPACITY);
+    }
   }
 }
 
@@ -91,6 +101,8 @@ __device__ __forceinline__ TallyPriv stage_priv(const DevProb &P, double *smem) 
 template <bool CE>
 __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, Soa S, u32 *stack, u64 *count,
                                                 u64 sec_start, u64 n_sec, u64 src_start, u64 n) {
+  // the host knows both cursors exactly here (it just synchronised): publish them for make_work
+  if (blockIdx.x == 0 && threadIdx.x == 0) { *R.src_next = src_start + (n - n_sec); *R.sec_head = sec_start + n_sec; }
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -113,7 +125,8 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
 // ---------------------------------------------------------------------------------- fused STEP (monolithic scheme)
 template <bool CE>
 __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in,
-                                              u32 *stack_out, u64 *count_out) {
+                                              u32 *stack_out, u64 *count_out, u64 *count_zero) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) *count_zero = 0;      // the stack the previous launch drained (3 rotating counters)
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
