@@ -168,6 +168,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
+  else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -385,6 +386,9 @@ static int run_async(tdr_problem *p, DevRun R) {
   p->diag.spills += h[40 + AC_SPILLS]; p->diag.fetches += h[40 + AC_FETCHES]; p->diag.make_work_calls += h[40 + AC_MAKEWORK];
   p->diag.events[1] += h[40 + AC_EVENTS]; p->diag.events[0] += R.src_total;
   int rc;
+  if ((int)h[C_COUNT - 1] == TDR_ELOST && h[40 + AC_DBG + 5])
+    return fail(TDR_ELOST, "async watchdog: warp %llu busy too long: link count %llu ev %llu nrun %llu nfree %llu iter %llu events %llu delta %lld outstanding %llu",
+                h[40 + AC_DBG], h[41 + AC_DBG], h[42 + AC_DBG], h[43 + AC_DBG], h[44 + AC_DBG], h[45 + AC_DBG], h[46 + AC_DBG], (long long)h[47 + AC_DBG], h[C_PENDING]);
   if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
   if (h[C_PENDING] != 0) return fail(TDR_ESTATE, "asynchronous scheme left %llu particles outstanding", h[C_PENDING]);
   return 0;

@@ -25,7 +25,7 @@
 
 
 struct GLink { u32 idx[32]; u32 count, ev, next, pad; };
-enum { AC_GWORK = 0, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_EVENTS, AC_COUNT = 8 };
+enum { AC_GWORK = 0, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_EVENTS, AC_DBG = 8, AC_COUNT = 16 };
 struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *actr; u64 *sec_flag; };
 
 template <class C>
@@ -55,8 +55,9 @@ __device__ __forceinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine
   }
 }
 
-__device__ __forceinline__ u32 q_pop(GLink *links, u64 *qs, u32 start) {
-  for (u32 a = 0; a < AQ; a++) {
+// A claimed queue looks like an empty one, so `rounds` full scans are made before the set is taken to be empty.
+__device__ __forceinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) {
+  for (u32 a = 0; a < AQ * rounds; a++) {
     u32 i = (start + a) % AQ;
     if (ld_vol(&qs[i]) == NULLQ) continue;
     u64 w = atomicExch(&qs[i], NULLQ);
@@ -118,7 +119,7 @@ __device__ __forceinline__ void spill_link(WarpCtx &w, int l, int fi) {
   const Stash &s = w.s;
   int c = s.cnt(l), e = s.ev(l);
   u32 g = NOLINK;
-  if (w.lane == 0) g = q_pop(w.A.links, w.A.q_empty, w.gw);
+  if (w.lane == 0) g = q_pop(w.A.links, w.A.q_empty, w.gw, 256);
   g = __shfl_sync(FULL, g, 0);
   if (g == NOLINK) { if (w.lane == 0) atomicExch(w.err, TDR_ECAPACITY); return; }
   if ((int)w.lane < c) w.A.links[g].idx[w.lane] = s.idx[l * 32 + w.lane];
@@ -139,7 +140,7 @@ __device__ __forceinline__ bool fetch_link(WarpCtx &w) {
   const Stash &s = w.s;
   if (s.nfree() == 0) return false;
   u32 g = NOLINK;
-  if (w.lane == 0 && ld_vol(&w.A.actr[AC_GWORK]) > 0) g = q_pop(w.A.links, w.A.q_work, w.gw);
+  if (w.lane == 0 && ld_vol(&w.A.actr[AC_GWORK]) > 0) g = q_pop(w.A.links, w.A.q_work, w.gw, 2);
   g = __shfl_sync(FULL, g, 0);
   if (g == NOLINK) return false;
   const int c = (int)*(volatile u32 *)&w.A.links[g].count, e = (int)*(volatile u32 *)&w.A.links[g].ev;
@@ -177,7 +178,9 @@ __device__ __forceinline__ void stash_insert(WarpCtx &w, int e, u32 value, bool 
     int pl = s.partial(e);
     if (pl < 0) {
       ensure_free_link(w);
-      if (s.nfree() == 0) return;                                 // error already flagged
+      const bool none = s.nfree() == 0;
+      __syncwarp();                                               // every lane has read the free count before lane 0 edits it
+      if (none) return;                                           // error already flagged
       if (w.lane == 0) { pl = s.freel(s.nfree() - 1); s.nfree() -= 1; s.partial(e) = pl; s.cnt(pl) = 0; s.ev(pl) = e; }
       __syncwarp();
       pl = s.partial(e);
@@ -270,6 +273,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
   u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
   bool starved = false;
   u32 n_events = 0, n_makework = 0, n_iter = 0;
+  const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
   for (;;) {
     int l = -1, fi = -1;
@@ -311,6 +315,15 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
       }
     }
     if (starved) { starved = false; if (w.lane == 0) atomicAdd(R.starved, ~0ull); }
+    if ((n_iter & 1023u) == 1023u) {                              // hard watchdog for a warp that stays busy
+      int ex = 0;
+      if (w.lane == 0 && global_ns() - t_start > 40 * deadline_ns) {
+        ex = 1; atomicExch(O.err, TDR_ELOST);
+        A.actr[AC_DBG] = w.gw; A.actr[AC_DBG + 1] = (u64)s.cnt(l); A.actr[AC_DBG + 2] = (u64)s.ev(l); A.actr[AC_DBG + 3] = (u64)s.nfull();
+        A.actr[AC_DBG + 4] = (u64)s.nfree(); A.actr[AC_DBG + 5] = n_iter; A.actr[AC_DBG + 6] = n_events; A.actr[AC_DBG + 7] = (u64)delta;
+      }
+      if (__shfl_sync(FULL, ex, 0)) break;
+    }
     // take the link out of the stash, then run its event on all lanes
     const int c = s.cnt(l), e = s.ev(l);
     const bool valid = (int)w.lane < c;
@@ -336,7 +349,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
     if (dm) {                                                   // only STEP / COLLIDE / SURFACE (or a lost particle) get here
       const u32 nc = __reduce_add_sync(FULL, (u32)nch);
       if (nc) push_children(O, R, &acc, p, nch, csrc);
-      delta += (i64)nc - (i64)__popc(dm);
+      delta += (R.kmode ? 0 : (i64)nc) - (i64)__popc(dm);     // k-mode children belong to the next generation
       if (make_work_async<CE>(P, mg, R, A, &acc, O.err, p, died)) { store_part<CE>(S, slot, p); next = first_ev; }
       else if (died && myfree == NOSLOT) myfree = slot;
     }

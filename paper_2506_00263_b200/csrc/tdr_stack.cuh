@@ -48,7 +48,7 @@ __device__ __forceinline__ void push_children(const DevOut &O, const DevRun &R, 
     else if (!R.sec_flag) { if (t - R.sec_head0 < R.sec_cap) R.sec[t % R.sec_cap] = s; else atomicExch(O.err, TDR_ECAPACITY); }
     else {                                                       // asynchronous scheme: publish with a ready flag
       const u64 k = t % R.sec_cap;
-      if (t - *(const volatile u64 *)R.sec_head < R.sec_cap - SEC_MARGIN) {
+      if ((i64)(t - *(const volatile u64 *)R.sec_head) < (i64)(R.sec_cap - SEC_MARGIN)) {     // the head may already be past t
         R.sec[k] = s; __threadfence(); *(volatile u64 *)&R.sec_flag[k] = t + 1;
       } else atomicExch(O.err, TDR_ECAPACITY);
     }
