@@ -31,6 +31,7 @@ struct tdr_problem {
   int blocks_per_sm = 0;                   // 0 = occupancy query
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
+  int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   int sync_every = 8;                      // stack scheme: remap iterations launched per counter read-back
   // workspace
@@ -168,6 +169,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
+  else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
@@ -365,7 +367,7 @@ template <bool CE, bool SPLIT>
 static int launch_async(tdr_problem *p, const DevRun &R, size_t smem) {
   int grid = grid_for(p, k_async<CE, SPLIT>, smem);
   KTimer t(p, true);
-  k_async<CE, SPLIT><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull);
+  k_async<CE, SPLIT><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull, (u32)p->slots_per_warp);
   return 0;
 }
 
@@ -373,7 +375,7 @@ template <bool CE>
 static int run_async(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
   const size_t smem = smem_bytes(p) + 8 * (size_t)STASH_WORDS(p->stash_links) * 4;
-  R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
+  R.defer_death = 1; R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
   k_async_init<<<1, 64, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
   LAUNCH_CHECK();

@@ -256,7 +256,7 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp
 
 // ---------------------------------------------------------------------------------- the persistent kernel
 template <bool CE, bool SPLIT>
-__global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns) {
+__global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
   i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
   u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
   bool starved = false;
-  u32 n_events = 0, n_makework = 0, n_iter = 0;
+  u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
   for (;;) {
@@ -282,7 +282,9 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
       if (source_has_work(R)) {
         // starved warp: every lane brings a slot (its own spare one, else a fresh one from the window) and claims work
         u32 need = __ballot_sync(FULL, myfree == NOSLOT);
+        if (fresh >= fresh_max) need = 0;                       // this warp's pool of slots is large enough
         if (need) {
+          fresh += 32;
           const int ld = __ffs(need) - 1; u64 b = ~0ull;
           if (w.lane == (u32)ld && ld_vol(R.slot_next) < R.W) b = atomicAdd(R.slot_next, (u64)__popc(need));
           b = __shfl_sync(FULL, b, ld);
@@ -335,6 +337,19 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
     }
     __syncwarp();
     Part p; int nch = 0, csrc = 0, next = NEXT_DEAD;
+    if (e == EV_SOURCE) {
+      // SOURCE event (make_work as an event): the link holds slots whose particles died.  Book the
+      // deaths 32 lanes wide, then refill the slots from the pending secondaries / the source.
+      u64 id = 0; u32 sg = 0, nc = 0;
+      if (valid) { id = S.id[slot]; sg = S.seg[slot]; nc = S.ncoll[slot]; }
+      record_deaths_warp(&acc, R, valid, id, sg, nc);
+      bool born = false;
+      if (source_has_work(R)) { born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, valid); n_makework++; }
+      if (born) store_part<CE>(S, slot, p);
+      else if (valid && myfree == NOSLOT) myfree = slot;
+      stash_insert(w, first_ev, slot, born);
+      continue;
+    }
     n_events += (u32)c;
     if (!SPLIT) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
     else switch (e) {
@@ -350,8 +365,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
       const u32 nc = __reduce_add_sync(FULL, (u32)nch);
       if (nc) push_children(O, R, &acc, p, nch, csrc);
       delta += (R.kmode ? 0 : (i64)nc) - (i64)__popc(dm);     // k-mode children belong to the next generation
-      if (make_work_async<CE>(P, mg, R, A, &acc, O.err, p, died)) { store_part<CE>(S, slot, p); next = first_ev; }
-      else if (died && myfree == NOSLOT) myfree = slot;
+      stash_insert(w, EV_SOURCE, slot, died);                   // the slot waits for the SOURCE event
     }
     if (!SPLIT) stash_insert(w, EV_STEP, slot, next == EV_STEP);
     else {

@@ -61,6 +61,7 @@ struct DevRun {
   // asynchronous scheme only: ready flags of the secondary ring (flag[t % cap] == t + 1 once record t is complete),
   // outstanding-particle count, bump allocator of window slots, count of starved warps, window size
   u64 *sec_flag, *outstanding, *slot_next, *starved; u64 W;
+  int defer_death;                            // deaths are booked by the SOURCE event (asynchronous scheme)
 };
 
 struct Part {
@@ -73,7 +74,7 @@ struct Part {
 // ---------------------------------------------------------------------------------- R1 Philox4x32-10
 struct Blk { u32 w0, w1, w2, w3; };
 
-__device__ __forceinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {
+__device__ __noinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {      // one copy in the instruction cache
 #pragma unroll
   for (int r = 0; r < 10; r++) {
     u32 h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;

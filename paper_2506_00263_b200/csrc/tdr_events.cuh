@@ -129,9 +129,10 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   p.seg += 1;                                                          // R3
   double dcoll = TDR_INF;
   if (St > 0.0) dcoll = -det_log(draw(seed, p.id, gen, p.seg, PUR_DIST, 0)) / St;
-  double dx = plane_dist(P.xp[p.ix], P.xp[p.ix + 1], p.x, p.u);
-  double dy = plane_dist(P.yp[p.iy], P.yp[p.iy + 1], p.y, p.v);
-  double dz = plane_dist(P.zp[p.iz], P.zp[p.iz + 1], p.z, p.w);
+  const double xl = P.xp[p.ix], xh = P.xp[p.ix + 1], yl = P.yp[p.iy], yh = P.yp[p.iy + 1], zl = P.zp[p.iz], zh = P.zp[p.iz + 1];
+  double dx = plane_dist(xl, xh, p.x, p.u);
+  double dy = plane_dist(yl, yh, p.y, p.v);
+  double dz = plane_dist(zl, zh, p.z, p.w);
   double dout = TDR_INF, din = TDR_INF;
   int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
   int nr = P.univ_nr[univ];
@@ -140,9 +141,12 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
     if (p.ring < nr) dout = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring], true);
     if (p.ring > 0) din = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring - 1], false);
   }
-  double dmx = plane_dist(P.mesh[0][p.mx], P.mesh[0][p.mx + 1], p.x, p.u);
-  double dmy = plane_dist(P.mesh[1][p.my], P.mesh[1][p.my + 1], p.y, p.v);
-  double dmz = plane_dist(P.mesh[2][p.mz], P.mesh[2][p.mz + 1], p.z, p.w);
+  // mesh planes: a mesh cell bounded by the very same plane values as the lattice cell gives the very same quotient
+  const double mxl = P.mesh[0][p.mx], mxh = P.mesh[0][p.mx + 1], myl = P.mesh[1][p.my], myh = P.mesh[1][p.my + 1];
+  const double mzl = P.mesh[2][p.mz], mzh = P.mesh[2][p.mz + 1];
+  double dmx = (mxl == xl && mxh == xh) ? dx : plane_dist(mxl, mxh, p.x, p.u);
+  double dmy = (myl == yl && myh == yh) ? dy : plane_dist(myl, myh, p.y, p.v);
+  double dmz = (mzl == zl && mzh == zh) ? dz : plane_dist(mzl, mzh, p.z, p.w);
   double ds = dx;
   if (dy < ds) ds = dy;
   if (dz < ds) ds = dz;
@@ -187,6 +191,7 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
 // ---------------------------------------------------------------------------------- death bookkeeping (D3)
 __device__ __forceinline__ void record_death(BlockAcc *a, const DevRun &R, const Part &p, int total_kind) {
   atomicAdd(&a->t64[total_kind], 1ull);
+  if (R.defer_death) return;                 // asynchronous scheme: the SOURCE event books the rest, 32 lanes wide
   atomicAdd(&a->t64[TDR_T_NSEG], (u64)p.seg);
   atomicAdd(&a->t64[TDR_T_NCOLL], (u64)p.ncoll);
   atomicAdd(&a->t64[TDR_T_NCROSS], (u64)(p.seg - p.ncoll));
@@ -195,6 +200,28 @@ __device__ __forceinline__ void record_death(BlockAcc *a, const DevRun &R, const
   if (R.hist_cap) {
     u64 k = atomicAdd(R.hist_count, 1ull);
     if (k < R.hist_cap) { R.hist_id[k] = p.id; R.hist_nseg[k] = p.seg; R.hist_ncoll[k] = p.ncoll; }
+  }
+}
+
+// the same bookkeeping for a whole link of dead particles (valid = lane holds one): warp-reduced, one atomic each
+__device__ __forceinline__ void record_deaths_warp(BlockAcc *a, const DevRun &R, bool valid, u64 id, u32 seg, u32 ncoll) {
+  const u32 lane = threadIdx.x & 31;
+  const u32 m = __ballot_sync(FULL, valid);
+  if (m == 0) return;
+  const u32 sseg = __reduce_add_sync(FULL, valid ? seg : 0u), scoll = __reduce_add_sync(FULL, valid ? ncoll : 0u);
+  u64 dg = 0;
+  if (valid) { Blk h = philox((u32)id, (u32)(id >> 32), ncoll, seg - ncoll, seg, 0x7D12u); dg = ((u64)h.w1 << 32) | h.w0; }
+  const u64 sdg = (u64)warp_sum_i64((i64)dg);
+  u64 base = 0;
+  if (lane == 0) {
+    atomicAdd(&a->t64[TDR_T_NSEG], (u64)sseg); atomicAdd(&a->t64[TDR_T_NCOLL], (u64)scoll);
+    atomicAdd(&a->t64[TDR_T_NCROSS], (u64)(sseg - scoll)); atomicAdd(&a->t64[TDR_T_DIGEST], sdg);
+    if (R.hist_cap) base = atomicAdd(R.hist_count, (u64)__popc(m));
+  }
+  if (R.hist_cap) {
+    base = __shfl_sync(FULL, base, 0);
+    const u64 k = base + __popc(m & ((1u << lane) - 1u));
+    if (valid && k < R.hist_cap) { R.hist_id[k] = id; R.hist_nseg[k] = seg; R.hist_ncoll[k] = ncoll; }
   }
 }
 

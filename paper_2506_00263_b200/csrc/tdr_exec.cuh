@@ -34,6 +34,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
       else if (flags & F_COLLIDE) alive = ev_collide<CE>(P, mg, R, acc, p, St, gi, f, nch, csrc);
       else alive = ev_surface(P, R, acc, p, flags);
       if (alive) store_part<CE>(S, slot, p);
+      else if (R.defer_death) { S.seg[slot] = p.seg; S.ncoll[slot] = p.ncoll; }
     }
     return alive ? EV_STEP : NEXT_DEAD;
   }
@@ -74,7 +75,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     if (alive) {
       S.u[slot] = p.u; S.v[slot] = p.v; S.w[slot] = p.w; S.ncoll[slot] = p.ncoll; S.loc1[slot] = pack_loc1(p);
       if (CE) S.E[slot] = p.E;
-    }
+    } else if (R.defer_death) S.ncoll[slot] = p.ncoll;
     return alive ? first_ev : NEXT_DEAD;
   }
   if (EV == EV_SURFACE) {

@@ -10,7 +10,7 @@ enum { C_SRC_NEXT = 0, C_SEC_TAIL, C_SEC_HEAD, C_BANK, C_HIST, C_NEXT_BANK, C_PE
        C_STACK0 = 8, /* C_STACK0..+7: stack counts */ C_COUNT = 16 };
 
 // event ids (split decomposition; async scheme)
-enum { EV_LOOKUP = 0, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_STEP, EV_FREE, EV_COUNT };
+enum { EV_LOOKUP = 0, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_STEP, EV_SOURCE, EV_COUNT };
 
 // asynchronous scheme: a claimed secondary may still be read this many records behind the tail, so the ring keeps
 // this much headroom (>= the number of resident threads, 148 x 2048)
