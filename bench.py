@@ -232,7 +232,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="both", choices=["stack", "async", "both"])
-    ap.add_argument("--decomposition", default="fused", choices=["fused", "split"])
+    ap.add_argument("--decomposition", default="fused", choices=["fused", "split", "hybrid"])
     ap.add_argument("--particles", type=int, default=1000000)
     ap.add_argument("--inactive", type=int, default=20)
     ap.add_argument("--active", type=int, default=50)

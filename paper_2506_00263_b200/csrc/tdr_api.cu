@@ -25,7 +25,7 @@ struct tdr_problem {
   int S = 24;
   // options
   int scheme = 0;                          // 0 stack, 1 async
-  int split = 0;                           // 0 fused, 1 split
+  int split = 0;                           // 0 fused, 1 split, 2 hybrid (step + collide events)
   u64 window = 1ull << 20;
   int stash_links = 8;
   int blocks_per_sm = 0;                   // 0 = occupancy query
@@ -163,7 +163,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   if (!p || !key || !value) return fail(TDR_EINVAL, "null argument");
   std::string k(key), v(value);
   if (k == "scheme") { if (v == "stack") p->scheme = 0; else if (v == "async") p->scheme = 1; else return fail(TDR_EINVAL, "scheme must be stack|async"); }
-  else if (k == "decomposition") { if (v == "fused") p->split = 0; else if (v == "split") p->split = 1; else return fail(TDR_EINVAL, "decomposition must be fused|split"); }
+  else if (k == "decomposition") { if (v == "fused") p->split = 0; else if (v == "split") p->split = 1; else if (v == "hybrid") p->split = 2; else return fail(TDR_EINVAL, "decomposition must be fused|split|hybrid"); }
   else if (k == "window") { long long w = atoll(value); if (w < 32) return fail(TDR_EINVAL, "window too small"); p->window = (u64)w; }
   else if (k == "stash_links") { int n = atoi(value); if (n < 8 || n > 64) return fail(TDR_EINVAL, "stash_links in [8,64]"); p->stash_links = n; }
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
@@ -315,11 +315,13 @@ static int run_stack(tdr_problem *p, DevRun R) {
   u64 n0 = R.src_total < W ? R.src_total : W;
   // fused: two index stacks, three rotating counters (in, out, the one to clear); split: one stack per event
   u64 it = 0;
-  if (!p->split) { if ((rc = source(p->stacks[0], ctr + C_STACK0, 0, n0))) return rc; }
+  const bool split = p->split == 1, hybrid = p->split == 2;
+  if (!split) { if ((rc = source(p->stacks[0], ctr + C_STACK0, 0, n0))) return rc; }
   else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, 0, n0))) return rc;
   u64 n_in = n0;
-  const int g_step = p->split ? 0 : grid_for(p, k_step<CE>, smem);
-  SplitGrids sg; if (p->split) split_grids<CE>(p, smem, sg);
+  const int g_step = split ? 0 : hybrid ? grid_for(p, k_step<CE, true>, smem) : grid_for(p, k_step<CE, false>, smem);
+  const int g_coll = hybrid ? grid_for(p, k_collide<CE>, smem) : 0;
+  SplitGrids sg; if (split) split_grids<CE>(p, smem, sg);
   for (;;) {
     R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
     // the out count never exceeds the in count (dead lanes are reborn in place), so n_in bounds every launch of
@@ -328,11 +330,20 @@ static int run_stack(tdr_problem *p, DevRun R) {
     u64 blocks64 = (n_in + 255) / 256; int cap_blocks = blocks64 > (1u << 30) ? (1 << 30) : (int)blocks64;
     if (cap_blocks < 1) cap_blocks = 1;
     for (int b = 0; b < batch; b++) {
-      if (!p->split) {
+      if (!split) {
         const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
+        u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // hybrid: collide-stack counters
+        const int g1 = g_step < cap_blocks ? g_step : cap_blocks;
         KTimer t(p, true);
-        k_step<CE><<<g_step < cap_blocks ? g_step : cap_blocks, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                                               p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr);
+        if (hybrid) {
+          k_step<CE, true><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+                                                  p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz);
+          k_collide<CE><<<g_coll < cap_blocks ? g_coll : cap_blocks, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[2], cc,
+                                                                                     p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
+          p->diag.kernel_launches++;
+        } else
+          k_step<CE, false><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+                                                   p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr);
         LAUNCH_CHECK(); p->diag.kernel_launches++;
       } else if ((rc = split_iteration<CE>(p, R, smem, sg, cap_blocks))) return rc;
       it++; p->diag.iterations++;
@@ -340,7 +351,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
     CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
     if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
-    const u64 alive = p->split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + it % 3];
+    const u64 alive = split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + it % 3];
     n_in = alive;
     h_sec_tail = h[C_SEC_TAIL];
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
@@ -350,7 +361,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
       if (pend + rem == 0) break;
       u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;
       R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
-      if (!p->split) { if ((rc = source(p->stacks[it & 1], ctr + C_STACK0 + it % 3, n_sec, n))) return rc; }
+      if (!split) { if ((rc = source(p->stacks[it & 1], ctr + C_STACK0 + it % 3, n_sec, n))) return rc; }
       else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, n_sec, n))) return rc;
       n_in = n;
     } else if (h[C_SEC_HEAD] != h_sec_head) {
@@ -363,11 +374,11 @@ static int run_stack(tdr_problem *p, DevRun R) {
 }
 
 // ---------------------------------------------------------------------------------- asynchronous scheme, one generation
-template <bool CE, bool SPLIT>
+template <bool CE, int MODE>
 static int launch_async(tdr_problem *p, const DevRun &R, size_t smem) {
-  int grid = grid_for(p, k_async<CE, SPLIT>, smem);
+  int grid = grid_for(p, k_async<CE, MODE>, smem);
   KTimer t(p, true);
-  k_async<CE, SPLIT><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull, (u32)p->slots_per_warp);
+  k_async<CE, MODE><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull, (u32)p->slots_per_warp);
   return 0;
 }
 
@@ -379,7 +390,7 @@ static int run_async(tdr_problem *p, DevRun R) {
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
   k_async_init<<<1, 64, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
   LAUNCH_CHECK();
-  if (p->split) launch_async<CE, true>(p, R, smem); else launch_async<CE, false>(p, R, smem);
+  if (p->split == 1) launch_async<CE, 1>(p, R, smem); else if (p->split == 2) launch_async<CE, 2>(p, R, smem); else launch_async<CE, 0>(p, R, smem);
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
   u64 *h = p->h_ctr;
   CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));

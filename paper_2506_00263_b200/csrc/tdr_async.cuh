@@ -41,7 +41,7 @@ __device__ __forceinline__ u64 ld_vol(const u64 *p) { return *(const volatile u6
 __device__ __forceinline__ u64 global_ns() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 
 // ---------------------------------------------------------------------------------- global queues (lane 0 only)
-__device__ __forceinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine) {
+__device__ __noinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine) {
   for (;;) {
     u64 cur = atomicExch(&qs[i], NULLQ);                         // claim whatever is there
     if (cur != NULLQ) {                                          // merge privately: cur ++ mine
@@ -56,7 +56,7 @@ __device__ __forceinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine
 }
 
 // A claimed queue looks like an empty one, so `rounds` full scans are made before the set is taken to be empty.
-__device__ __forceinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) {
+__device__ __noinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) {
   for (u32 a = 0; a < AQ * rounds; a++) {
     u32 i = (start + a) % AQ;
     if (ld_vol(&qs[i]) == NULLQ) continue;
@@ -255,7 +255,8 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp
 }
 
 // ---------------------------------------------------------------------------------- the persistent kernel
-template <bool CE, bool SPLIT>
+// MODE: 0 fused (monolithic step), 1 split (five events), 2 hybrid (step with the collision as its own event)
+template <bool CE, int MODE>
 __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
@@ -268,6 +269,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
   w.s.idx = stash_mem; w.s.meta = (int *)(stash_mem + 32 * L); w.s.L = L;
   stash_init(w.s, w.lane);
   const Stash &s = w.s;
+  constexpr bool SPLIT = MODE == 1;
   const int first_ev = SPLIT ? EV_LOOKUP : EV_STEP;
   i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
   u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
@@ -351,7 +353,11 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
       continue;
     }
     n_events += (u32)c;
-    if (!SPLIT) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
+    if (MODE == 0) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
+    else if (MODE == 2) {
+      if (e == EV_STEP) next = exec_event<CE, EV_STEP, true>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
+      else next = exec_event<CE, EV_COLLIDE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
+    }
     else switch (e) {
       case EV_LOOKUP: next = exec_event<CE, EV_LOOKUP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
       case EV_MOVE: next = exec_event<CE, EV_MOVE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev); break;
@@ -367,7 +373,8 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
       delta += (R.kmode ? 0 : (i64)nc) - (i64)__popc(dm);     // k-mode children belong to the next generation
       stash_insert(w, EV_SOURCE, slot, died);                   // the slot waits for the SOURCE event
     }
-    if (!SPLIT) stash_insert(w, EV_STEP, slot, next == EV_STEP);
+    if (MODE == 0) stash_insert(w, EV_STEP, slot, next == EV_STEP);
+    else if (MODE == 2) { stash_insert(w, EV_STEP, slot, next == EV_STEP); if (e == EV_STEP) stash_insert(w, EV_COLLIDE, slot, next == EV_COLLIDE); }
     else {
       if (e == EV_LOOKUP) stash_insert(w, EV_MOVE, slot, next == EV_MOVE);
       else if (e == EV_MOVE) stash_insert(w, EV_TALLY, slot, next == EV_TALLY);

@@ -217,6 +217,7 @@ __device__ __forceinline__ double dist_cyl(double X, double Y, double u, double 
 
 __device__ __forceinline__ int find_bin(const double *pl, int n, double x) {   // G2
   int k = 0;
+#pragma unroll 1
   for (int i = 1; i < n; i++) if (pl[i] <= x) k = i;
   return k;
 }

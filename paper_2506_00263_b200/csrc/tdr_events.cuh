@@ -7,12 +7,23 @@
 // flags produced by MOVE
 enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512 };
 
-// per-block accumulators in shared memory, flushed once per kernel (finalize hook)
+// per-block accumulators in shared memory, flushed once per kernel (finalize hook).  Every 64-bit sum
+// is two 32-bit words updated with native shared atomics: the carry out of the low word goes to the high word, so
+// the sum is exact mod 2^64 (a 64-bit shared atomicAdd would be a compare-and-swap loop).
 struct BlockAcc {
-  u64 t64[TDR_T_COUNT];     // totals (nseg/ncoll/digest/nsites use 64-bit; others small)
+  u32 lo[TDR_T_COUNT + 2], hi[TDR_T_COUNT + 2];     // totals, then P and Pc
   u32 leak[6];
-  i64 P, Pc;
 };
+#define ACC_P TDR_T_COUNT
+#define ACC_PC (TDR_T_COUNT + 1)
+
+__device__ __forceinline__ void add64_shared(u32 *lo, u32 *hi, u32 k, u64 val) {
+  u32 vl = (u32)val, vh = (u32)(val >> 32);
+  u32 old = atomicAdd(&lo[k], vl);
+  vh += (u32)(((u64)old + vl) >> 32);
+  if (vh) atomicAdd(&hi[k], vh);
+}
+__device__ __forceinline__ void acc_add(BlockAcc *a, int kind, u64 v) { add64_shared(a->lo, a->hi, (u32)kind, v); }
 
 __device__ __forceinline__ void acc_init(BlockAcc *a) {
   for (int i = threadIdx.x; i < (int)(sizeof(BlockAcc) / 4); i += blockDim.x) ((u32 *)a)[i] = 0;
@@ -29,13 +40,13 @@ __device__ __forceinline__ i64 warp_sum_i64(i64 v) {      // exact: 3 limbs of <
 
 __device__ __forceinline__ void acc_flush(BlockAcc *a, const DevOut &o, i64 P, i64 Pc) {
   i64 wp = warp_sum_i64(P), wpc = warp_sum_i64(Pc);      // two's complement limbs: exact mod 2^64
-  if ((threadIdx.x & 31) == 0) { atomicAdd((u64 *)&a->P, (u64)wp); atomicAdd((u64 *)&a->Pc, (u64)wpc); }
+  if ((threadIdx.x & 31) == 0) { acc_add(a, ACC_P, (u64)wp); acc_add(a, ACC_PC, (u64)wpc); }
   __syncthreads();
   int t = threadIdx.x;
-  if (t < TDR_T_COUNT) { if (a->t64[t]) atomicAdd(&o.totals[t], a->t64[t]); }
-  else if (t < TDR_T_COUNT + 6) { if (a->leak[t - TDR_T_COUNT]) atomicAdd(&o.leak[t - TDR_T_COUNT], (u64)a->leak[t - TDR_T_COUNT]); }
-  else if (t == TDR_T_COUNT + 6) { if (a->P) atomicAdd(&o.PPc[0], (u64)a->P); }
-  else if (t == TDR_T_COUNT + 7) { if (a->Pc) atomicAdd(&o.PPc[1], (u64)a->Pc); }
+  if (t < TDR_T_COUNT + 2) {
+    u64 v = ((u64)a->hi[t] << 32) + a->lo[t];
+    if (v) atomicAdd(t < TDR_T_COUNT ? &o.totals[t] : &o.PPc[t - TDR_T_COUNT], v);
+  } else if (t < TDR_T_COUNT + 8) { if (a->leak[t - TDR_T_COUNT - 2]) atomicAdd(&o.leak[t - TDR_T_COUNT - 2], (u64)a->leak[t - TDR_T_COUNT - 2]); }
 }
 
 // Block-private tallies in shared memory (finalize hook): used when the tally has few bins, where
@@ -51,12 +62,7 @@ __device__ __forceinline__ TallyPriv priv_init(const DevProb &P, void *mem) {
   for (int i = threadIdx.x; i < 4 * t.n; i += blockDim.x) w[i] = 0;
   return t;
 }
-__device__ __forceinline__ void priv_add(u32 *lo, u32 *hi, u32 bin, u64 val) {
-  u32 vl = (u32)val, vh = (u32)(val >> 32);
-  u32 old = atomicAdd(&lo[bin], vl);
-  vh += (u32)(((u64)old + vl) >> 32);
-  if (vh) atomicAdd(&hi[bin], vh);
-}
+__device__ __forceinline__ void priv_add(u32 *lo, u32 *hi, u32 bin, u64 val) { add64_shared(lo, hi, bin, val); }
 __device__ __forceinline__ void priv_flush(const TallyPriv &t, const DevOut &o) {   // after __syncthreads()
   for (int i = threadIdx.x; i < t.n; i += blockDim.x) {
     u64 f = ((u64)t.flux_hi[i] << 32) | t.flux_lo[i], c = ((u64)t.coll_hi[i] << 32) | t.coll_lo[i];
@@ -190,13 +196,13 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
 
 // ---------------------------------------------------------------------------------- death bookkeeping (D3)
 __device__ __forceinline__ void record_death(BlockAcc *a, const DevRun &R, const Part &p, int total_kind) {
-  atomicAdd(&a->t64[total_kind], 1ull);
+  acc_add(a, total_kind, 1ull);
   if (R.defer_death) return;                 // asynchronous scheme: the SOURCE event books the rest, 32 lanes wide
-  atomicAdd(&a->t64[TDR_T_NSEG], (u64)p.seg);
-  atomicAdd(&a->t64[TDR_T_NCOLL], (u64)p.ncoll);
-  atomicAdd(&a->t64[TDR_T_NCROSS], (u64)(p.seg - p.ncoll));
+  acc_add(a, TDR_T_NSEG, (u64)p.seg);
+  acc_add(a, TDR_T_NCOLL, (u64)p.ncoll);
+  acc_add(a, TDR_T_NCROSS, (u64)(p.seg - p.ncoll));
   Blk h = philox((u32)p.id, (u32)(p.id >> 32), p.ncoll, p.seg - p.ncoll, p.seg, 0x7D12u);
-  atomicAdd(&a->t64[TDR_T_DIGEST], ((u64)h.w1 << 32) | h.w0);
+  acc_add(a, TDR_T_DIGEST, ((u64)h.w1 << 32) | h.w0);
   if (R.hist_cap) {
     u64 k = atomicAdd(R.hist_count, 1ull);
     if (k < R.hist_cap) { R.hist_id[k] = p.id; R.hist_nseg[k] = p.seg; R.hist_ncoll[k] = p.ncoll; }
@@ -214,8 +220,8 @@ __device__ __forceinline__ void record_deaths_warp(BlockAcc *a, const DevRun &R,
   const u64 sdg = (u64)warp_sum_i64((i64)dg);
   u64 base = 0;
   if (lane == 0) {
-    atomicAdd(&a->t64[TDR_T_NSEG], (u64)sseg); atomicAdd(&a->t64[TDR_T_NCOLL], (u64)scoll);
-    atomicAdd(&a->t64[TDR_T_NCROSS], (u64)(sseg - scoll)); atomicAdd(&a->t64[TDR_T_DIGEST], sdg);
+    acc_add(a, TDR_T_NSEG, (u64)sseg); acc_add(a, TDR_T_NCOLL, (u64)scoll);
+    acc_add(a, TDR_T_NCROSS, (u64)(sseg - scoll)); acc_add(a, TDR_T_DIGEST, sdg);
     if (R.hist_cap) base = atomicAdd(R.hist_count, (u64)__popc(m));
   }
   if (R.hist_cap) {
@@ -242,7 +248,7 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
     nu = row[4]; child_src = mat;
     if (kind == 0) {
       p.g = sample_cdf(row + 5, P.G, draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0));
-      if (iso_dir(seed, p.id, gen, p.seg, p.u, p.v, p.w)) atomicAdd(&acc->t64[TDR_T_NDIRFAIL], 1ull);
+      if (iso_dir(seed, p.id, gen, p.seg, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
       return true;
     }
   } else {
@@ -267,7 +273,7 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
   double nu_eff = R.kmode ? nu / R.k_prev : nu;
   int n = (int)floor(nu_eff + draw(seed, p.id, gen, p.seg, PUR_MULT, 0));
   if (n > 64) n = 64;
-  if (!R.kmode && p.depth >= 200) { atomicAdd(&acc->t64[TDR_T_NDROPPED], (u64)n); n = 0; }
+  if (!R.kmode && p.depth >= 200) { acc_add(acc, TDR_T_NDROPPED, (u64)n); n = 0; }
   n_children = n;
   record_death(acc, R, p, TDR_T_NFIS);
   return false;
@@ -311,14 +317,14 @@ __device__ __forceinline__ void birth_common(const DevProb &P, const double *mg,
                                              int src, bool from_site) {
   p.seg = 0; p.ncoll = 0; p.E = 0.0; p.g = 0;
   if (!from_site && P.src_dir_kind == 1) { p.u = P.src_dir[0]; p.v = P.src_dir[1]; p.w = P.src_dir[2]; }
-  else if (iso_dir(R.seed, p.id, R.gen, 0, p.u, p.v, p.w)) atomicAdd(&acc->t64[TDR_T_NDIRFAIL], 1ull);
+  else if (iso_dir(R.seed, p.id, R.gen, 0, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
   if (from_site) {
     if (!CE) p.g = sample_cdf(mg + P.n_mat * P.G * MGROW(P.G) + src * P.G, P.G, draw(R.seed, p.id, R.gen, 0, PUR_ENERGY, 0));
     else p.E = watt(R.seed, p.id, R.gen, P.wa[src], P.wb[src]);
   } else if (P.src_energy_kind == 0) p.g = P.src_index;
   else if (P.src_energy_kind == 1) p.E = P.src_energy;
   else p.E = watt(R.seed, p.id, R.gen, P.wa[P.src_index], P.wb[P.src_index]);
-  atomicAdd(&acc->t64[TDR_T_NBORN], 1ull);
+  acc_add(acc, TDR_T_NBORN, 1ull);
 }
 
 template <bool CE>

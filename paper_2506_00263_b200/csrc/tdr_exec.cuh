@@ -15,7 +15,7 @@ __device__ __forceinline__ void load_loc_energy(const Soa &S, u32 i, Part &p) {
 }
 
 // returns the next event of this lane's particle (NEXT_DEAD if it died or the lane is idle)
-template <bool CE, int EV>
+template <bool CE, int EV, bool HYBRID = false>
 __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, const DevOut &O, const TallyPriv &tp, const DevRun &R, const Soa &S,
                                           BlockAcc *acc, u32 slot, bool valid, Part &p, int &nch, int &csrc,
                                           i64 &accP, i64 &accPc, int first_ev) {
@@ -31,7 +31,14 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     bool alive = false;
     if (valid) {
       if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
-      else if (flags & F_COLLIDE) alive = ev_collide<CE>(P, mg, R, acc, p, St, gi, f, nch, csrc);
+      else if (flags & F_COLLIDE) {
+        if (HYBRID) {                                     // hybrid scheme: collisions are their own event (uniform warps)
+          S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; S.s_sigt[slot] = St;
+          if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
+          return EV_COLLIDE;
+        }
+        alive = ev_collide<CE>(P, mg, R, acc, p, St, gi, f, nch, csrc);
+      }
       else alive = ev_surface(P, R, acc, p, flags);
       if (alive) store_part<CE>(S, slot, p);
       else if (R.defer_death) { S.seg[slot] = p.seg; S.ncoll[slot] = p.ncoll; }

@@ -41,6 +41,31 @@ __global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun R, So
   if (EV == EV_TALLY) priv_flush(tp, O);
 }
 
+// hybrid scheme, second kernel of a remap iteration: the COLLIDE event on the collide stack; survivors (and lanes
+// reborn by make_work) join the step stack the preceding k_step<CE, true> launch was pushing to.
+template <bool CE>
+__global__ void __launch_bounds__(256) k_collide(DevProb P, DevOut O, DevRun R, Soa S, const u32 *cstack, const u64 *ccount,
+                                                 u32 *stack_out, u64 *count_out) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  const TallyPriv tp = stage_priv(P, smem);
+  acc_init(&acc);
+  const u64 n_in = *ccount;
+  i64 accP = 0, accPc = 0;
+  for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_in; i0 += (u64)gridDim.x * blockDim.x) {
+    u64 i = i0 + threadIdx.x;
+    bool valid = i < n_in;
+    u32 slot = valid ? cstack[i] : 0;
+    Part p; int nch, csrc;
+    int next = exec_event<CE, EV_COLLIDE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, EV_STEP);
+    push_children(O, R, &acc, p, nch, csrc);
+    if (make_work<CE>(P, mg, R, &acc, p, valid && next == NEXT_DEAD)) { store_part<CE>(S, slot, p); next = EV_STEP; }
+    stack_push(stack_out, count_out, slot, next == EV_STEP);
+  }
+  acc_flush(&acc, O, accP, accPc);
+}
+
 struct SplitGrids { int g[EV_COUNT]; };
 
 // host side -----------------------------------------------------------------------------------------------

@@ -39,7 +39,7 @@ __device__ __forceinline__ void push_children(const DevOut &O, const DevRun &R, 
   for (int o = 1; o < 32; o <<= 1) { u32 t = __shfl_up_sync(FULL, incl, o); if (lane >= (u32)o) incl += t; }
   u32 excl = incl - (u32)n;
   u64 base = 0;
-  if (lane == 0) { base = atomicAdd(R.kmode ? R.bank_count : R.sec_tail, (u64)total); atomicAdd(&acc->t64[TDR_T_NSITES], (u64)total); }
+  if (lane == 0) { base = atomicAdd(R.kmode ? R.bank_count : R.sec_tail, (u64)total); acc_add(acc, TDR_T_NSITES, (u64)total); }
   base = __shfl_sync(FULL, base, 0);
   for (int c = 0; c < n; c++) {
     u64 t = base + excl + c;
@@ -123,10 +123,16 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
 }
 
 // ---------------------------------------------------------------------------------- fused STEP (monolithic scheme)
-template <bool CE>
+// HYBRID: a particle that collides is not processed here; it is pushed onto the collide stack (cstack) and the
+// collision runs as its own event in k_collide, where every lane of a warp takes the same path.
+template <bool CE, bool HYBRID>
 __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in,
-                                              u32 *stack_out, u64 *count_out, u64 *count_zero) {
-  if (blockIdx.x == 0 && threadIdx.x == 0) *count_zero = 0;      // the stack the previous launch drained (3 rotating counters)
+                                              u32 *stack_out, u64 *count_out, u64 *count_zero,
+                                              u32 *cstack, u64 *ccount, u64 *ccount_zero) {
+  if (blockIdx.x == 0 && threadIdx.x == 0) {       // the stacks the previous launches drained (rotating counters)
+    *count_zero = 0;
+    if (HYBRID) *ccount_zero = 0;
+  }
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -146,16 +152,23 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
       ev_move(P, R.seed, R.gen, p, St, d, flags);
     }
     ev_tally<CE>(P, O, tp, R, p, valid && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
-    bool alive = false; int nch = 0, csrc = 0;
+    bool alive = false, to_collide = false; int nch = 0, csrc = 0;
     if (valid) {
       if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
-      else if (flags & F_COLLIDE) alive = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+      else if (flags & F_COLLIDE) {
+        if (HYBRID) {
+          S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; S.s_sigt[slot] = St;
+          if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
+          to_collide = true;
+        } else alive = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+      }
       else alive = ev_surface(P, R, &acc, p, flags);
     }
-    push_children(O, R, &acc, p, nch, csrc);
-    if (make_work<CE>(P, mg, R, &acc, p, valid && !alive)) alive = true;
+    if (!HYBRID) push_children(O, R, &acc, p, nch, csrc);
+    if (make_work<CE>(P, mg, R, &acc, p, valid && !alive && !to_collide)) alive = true;
     if (alive) store_part<CE>(S, slot, p);
     stack_push(stack_out, count_out, slot, alive);
+    if (HYBRID) stack_push(cstack, ccount, slot, to_collide);
   }
   acc_flush(&acc, O, accP, accPc);
   priv_flush(tp, O);

@@ -9,7 +9,7 @@ from tests.parity import assert_same, run_both
 
 pytestmark = pytest.mark.gpu
 
-SCHEMES = [("stack", "fused"), ("stack", "split"), ("async", "fused"), ("async", "split")]
+SCHEMES = [("stack", "fused"), ("stack", "split"), ("stack", "hybrid"), ("async", "fused"), ("async", "split"), ("async", "hybrid")]
 
 
 def small_cases():
