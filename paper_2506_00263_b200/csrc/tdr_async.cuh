@@ -256,8 +256,11 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp
 
 // ---------------------------------------------------------------------------------- the persistent kernel
 // MODE: 0 fused (monolithic step), 1 split (five events), 2 hybrid (step with the collision as its own event)
+#ifndef TDR_ASYNC_MINB
+#define TDR_ASYNC_MINB 2
+#endif
 template <bool CE, int MODE>
-__global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max) {
+__global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -274,7 +277,7 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
   i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
   u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
   bool starved = false;
-  u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0;
+  u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
   for (;;) {
@@ -314,11 +317,11 @@ __global__ void __launch_bounds__(256) k_async(DevProb P, DevOut O, DevRun R, So
         out = __shfl_sync(FULL, out, 0); er = __shfl_sync(FULL, er, 0);
         if (out == 0 || er != 0) break;
         if (!starved) { starved = true; if (w.lane == 0) { atomicAdd(R.starved, 1ull); t_idle = global_ns(); } }
-        __nanosleep(500);
+        __nanosleep(backoff); if (backoff < 8000) backoff += backoff;      // idle warps leave the issue slots to the others
         continue;
       }
     }
-    if (starved) { starved = false; if (w.lane == 0) atomicAdd(R.starved, ~0ull); }
+    if (starved) { starved = false; backoff = 250; if (w.lane == 0) atomicAdd(R.starved, ~0ull); }
     if ((n_iter & 1023u) == 1023u) {                              // hard watchdog for a warp that stays busy
       int ex = 0;
       if (w.lane == 0 && global_ns() - t_start > 40 * deadline_ns) {

@@ -190,28 +190,24 @@ __device__ __forceinline__ void scatter_ce(u64 seed, u32 gen, Part &p, double A)
 }
 
 // ---------------------------------------------------------------------------------- G3 / G4 distances
+// Both are written without branches so that a warp issues ONE division (and one square root) whatever the signs
+// of its lanes' direction components; the selected operands and hence the quotients are those of G3 / G4.
 __device__ __forceinline__ double plane_dist(double lo, double hi, double x, double c) {
-  if (c > 0.0) return (hi - x) / c;
-  if (c < 0.0) return (lo - x) / c;
-  return TDR_INF;
+  const double pl = c > 0.0 ? hi : lo;
+  const double d = (pl - x) / c;
+  return c != 0.0 ? d : TDR_INF;
 }
 
 __device__ __forceinline__ double dist_cyl(double X, double Y, double u, double v, double R, bool inside) {
-  double a = u * u + v * v;
-  if (a == 0.0) return TDR_INF;
-  double b = X * u + Y * v;
-  double c = (X * X + Y * Y) - R * R;
-  double disc = b * b - a * c;
-  double d;
-  if (inside) {
-    if (disc < 0.0) disc = 0.0;
-    d = (-b + sqrt(disc)) / a;
-  } else {
-    if (b >= 0.0) return TDR_INF;
-    if (disc <= 0.0) return TDR_INF;
-    d = (-b - sqrt(disc)) / a;
-  }
+  const double a = u * u + v * v;
+  const double b = X * u + Y * v;
+  const double c = (X * X + Y * Y) - R * R;
+  const double disc = b * b - a * c;
+  const double sq = sqrt(disc < 0.0 ? 0.0 : disc);
+  double d = (-b + (inside ? sq : -sq)) / a;          // x - y is x + (-y) exactly
   if (d < 0.0) d = 0.0;
+  if (!inside && (b >= 0.0 || disc <= 0.0)) d = TDR_INF;
+  if (a == 0.0) d = TDR_INF;
   return d;
 }
 
@@ -230,9 +226,10 @@ __device__ __forceinline__ int locate_ring(const DevProb &P, int univ, double X,
 }
 
 __device__ __forceinline__ int sample_cdf(const double *cdf, int n, double xi) {   // X1
-  double t = xi * cdf[n - 1];
-  for (int k = 0; k < n; k++) if (t < cdf[k]) return k;
-  return n - 1;
+  const double t = xi * cdf[n - 1];
+  int k = n - 1;                                      // first index with t < cdf[k], else the last: no early exit
+  for (int j = n - 2; j >= 0; j--) if (t < cdf[j]) k = j;
+  return k;
 }
 
 // ---------------------------------------------------------------------------------- SoA load / store

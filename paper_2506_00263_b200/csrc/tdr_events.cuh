@@ -144,8 +144,12 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   int nr = P.univ_nr[univ];
   if (nr > 0) {
     double X = p.x - P.cx[p.ix], Y = p.y - P.cy[p.iy];
-    if (p.ring < nr) dout = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring], true);
-    if (p.ring > 0) din = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring - 1], false);
+    // a lane needs the cylinder outside it, the one inside it, or both; the first of them is computed by every lane
+    // in one instruction sequence (outward for one lane, inward for its neighbour), the second only between two rings
+    const bool out1 = p.ring < nr;
+    const double d1 = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + (out1 ? p.ring : p.ring - 1)], out1);
+    if (out1) dout = d1; else din = d1;
+    if (out1 && p.ring > 0) din = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring - 1], false);
   }
   // mesh planes: a mesh cell bounded by the very same plane values as the lattice cell gives the very same quotient
   const double mxl = P.mesh[0][p.mx], mxh = P.mesh[0][p.mx + 1], myl = P.mesh[1][p.my], myh = P.mesh[1][p.my + 1];
