@@ -118,8 +118,11 @@ typedef struct tdr_problem tdr_problem;
 
 /* Copy the problem to the device, derive tables (MG cdfs, CE hash).  TDR_EINVAL on bad input. */
 int tdr_init_problem(const tdr_geometry *, const tdr_materials *, const tdr_xs_tables *, tdr_problem **out);
-/* keys: "scheme" = stack|async; "decomposition" = fused|split; "window" = particles in flight;
- * "stash_links" (async, links per warp); "blocks_per_sm"; "keep_history" = 0|1. */
+/* keys: "scheme" = stack|async; "decomposition" = fused|split|hybrid; "window" = particles in flight;
+ * "stash_links" (async, links per warp, 8..64); "slots_per_warp" (async); "sync_every" (stack: remap iterations per
+ * counter read-back); "blocks_per_sm"; "keep_history" = 0|1; "time_kernels" = 0|1; "idle_timeout_s" (async watchdog);
+ * "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs).
+ * decomposition = fused (monolithic step) | split (five events) | hybrid (step + collide). */
 int tdr_set_option(tdr_problem *, const char *key, const char *value);
 int tdr_workspace_bytes(const tdr_problem *, uint64_t n_particles, uint64_t *bytes);
 /* device_ptr: DEVICE memory of at least `bytes` (256-byte aligned); cuda_stream: cudaStream_t. */

@@ -4,14 +4,15 @@
   workloads  seeded synthetic inputs (shared with the test oracle; no method arithmetic)
   tdr        ctypes binding of libtdr.so (loads the CUDA library; no CPU fallback)
   build      in-tree nvcc build
+  shard      multi-GPU plumbing: id-range sharding of a fixed source, int64 all-reduce of tallies
 """
 from . import workloads  # noqa: F401
 
-__all__ = ["workloads", "tdr", "build"]
+__all__ = ["workloads", "tdr", "build", "shard"]
 
 
 def __getattr__(name):
-    if name in ("tdr", "build"):
+    if name in ("tdr", "build", "shard"):
         import importlib
         return importlib.import_module("." + name, __name__)
     raise AttributeError(name)

@@ -33,6 +33,7 @@ struct tdr_problem {
   int time_kernels = 0;
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
+  u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
   int sync_every = 8;                      // stack scheme: remap iterations launched per counter read-back
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
@@ -171,6 +172,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "time_kernels") p->time_kernels = atoi(value);
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
+  else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -449,6 +451,7 @@ int tdr_run_fixed_source(tdr_problem *p, uint64_t n, uint64_t seed) {
   RunClock clk(p->stream);
   DevRun R; memset(&R, 0, sizeof R);
   R.seed = seed; R.gen = 0; R.kmode = 0; R.active = 1; R.k_prev = 1.0; R.src_sites = 0; R.sites = nullptr; R.src_total = n;
+  R.id_offset = p->id_offset;
   bool keep = p->keep_history < 0 ? n <= 2000000 : p->keep_history != 0;
   R.hist_cap = keep ? p->hist_cap : 0;
   if ((rc = run_generation(p, R))) return rc;

@@ -61,6 +61,7 @@ struct DevRun {
   // asynchronous scheme only: ready flags of the secondary ring (flag[t % cap] == t + 1 once record t is complete),
   // outstanding-particle count, bump allocator of window slots, count of starved warps, window size
   u64 *sec_flag, *outstanding, *slot_next, *starved; u64 W;
+  u64 id_offset;                              // first source id of this run (multi-GPU sharding of a fixed source)
   int defer_death;                            // deaths are booked by the SOURCE event (asynchronous scheme)
 };
 
@@ -194,8 +195,12 @@ __device__ __forceinline__ void scatter_ce(u64 seed, u32 gen, Part &p, double A)
 // of its lanes' direction components; the selected operands and hence the quotients are those of G3 / G4.
 __device__ __forceinline__ double plane_dist(double lo, double hi, double x, double c) {
   const double pl = c > 0.0 ? hi : lo;
-  const double d = (pl - x) / c;
-  return c != 0.0 ? d : TDR_INF;
+  const double num = pl - x;
+  // an infinite plane or a zero direction component gives +inf (G3) without entering the division: infinite or
+  // zero operands would send the whole warp through the slow path of the software fp64 division
+  const bool ok = (c != 0.0) && (fabs(num) < TDR_INF);
+  const double d = (ok ? num : 1.0) / (ok ? c : 1.0);
+  return ok ? d : TDR_INF;
 }
 
 __device__ __forceinline__ double dist_cyl(double X, double Y, double u, double v, double R, bool inside) {

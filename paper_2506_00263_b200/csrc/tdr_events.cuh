@@ -189,7 +189,8 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
     }
   }
   bool collide = valid && (flags & F_COLLIDE);
-  if (R.kmode && valid) { accP += fixp(d * nsf, P.scale); if (collide) accPc += fixp(nsf / St, P.scale); }
+  // (0/St = 0 scores nothing, and a zero numerator would take the slow path of the software division)
+  if (R.kmode && valid) { accP += fixp(d * nsf, P.scale); if (collide && nsf != 0.0) accPc += fixp(nsf / St, P.scale); }
   if (R.active) {
     u64 bin = 0;
     if (e >= 0) bin = ((((u64)p.mz * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;
@@ -333,10 +334,10 @@ __device__ __forceinline__ void birth_common(const DevProb &P, const double *mg,
 
 template <bool CE>
 __device__ __forceinline__ void birth_primary(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, u64 i) {
-  p.id = i; p.depth = 0;
+  p.id = i + R.id_offset; p.depth = 0;         // id_offset: this GPU's share of a source sharded by contiguous id ranges
   if (P.src_kind == 0) { p.x = P.src_lo[0]; p.y = P.src_lo[1]; p.z = P.src_lo[2]; }
   else {
-    Blk b0 = rng_block(R.seed, i, R.gen, 0, PUR_POS, 0), b1 = rng_block(R.seed, i, R.gen, 0, PUR_POS, 1);
+    Blk b0 = rng_block(R.seed, p.id, R.gen, 0, PUR_POS, 0), b1 = rng_block(R.seed, p.id, R.gen, 0, PUR_POS, 1);
     p.x = P.src_lo[0] + blk_even(b0) * (P.src_hi[0] - P.src_lo[0]);
     p.y = P.src_lo[1] + blk_odd(b0) * (P.src_hi[1] - P.src_lo[1]);
     p.z = P.src_lo[2] + blk_even(b1) * (P.src_hi[2] - P.src_lo[2]);
