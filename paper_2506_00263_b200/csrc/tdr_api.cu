@@ -31,6 +31,7 @@ struct tdr_problem {
   int blocks_per_sm = 0;                   // 0 = occupancy query
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
+  int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
@@ -170,6 +171,8 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
+  else if (k == "lockstep") p->lockstep = atoi(value) != 0;
+  else if (k == "async_threads") { int n = atoi(value); if (n != 128 && n != 256 && n != 512) return fail(TDR_EINVAL, "async_threads in {128,256,512}"); p->async_threads = n; }
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
@@ -377,22 +380,24 @@ static int run_stack(tdr_problem *p, DevRun R) {
 
 // ---------------------------------------------------------------------------------- asynchronous scheme, one generation
 template <bool CE, int MODE>
-static int launch_async(tdr_problem *p, const DevRun &R, size_t smem) {
-  int grid = grid_for(p, k_async<CE, MODE>, smem);
+static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int threads) {
+  int grid = grid_for(p, k_async<CE, MODE>, smem, threads);
   KTimer t(p, true);
-  k_async<CE, MODE><<<grid, 256, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull, (u32)p->slots_per_warp);
+  k_async<CE, MODE><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
+                                                        (u32)p->slots_per_warp, p->lockstep);
   return 0;
 }
 
 template <bool CE>
 static int run_async(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
-  const size_t smem = smem_bytes(p) + 8 * (size_t)STASH_WORDS(p->stash_links) * 4;
+  const int threads = p->async_threads;
+  const size_t smem = smem_bytes(p) + (threads / 32) * (size_t)STASH_WORDS(p->stash_links) * 4;
   R.defer_death = 1; R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
   k_async_init<<<1, 64, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
   LAUNCH_CHECK();
-  if (p->split == 1) launch_async<CE, 1>(p, R, smem); else if (p->split == 2) launch_async<CE, 2>(p, R, smem); else launch_async<CE, 0>(p, R, smem);
+  if (p->split == 1) launch_async<CE, 1>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2>(p, R, smem, threads); else launch_async<CE, 0>(p, R, smem, threads);
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
   u64 *h = p->h_ctr;
   CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));

@@ -245,13 +245,18 @@ __device__ __forceinline__ bool make_work_async(const DevProb &P, const double *
   return reborn;
 }
 
-__device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp-uniform
-  bool yes = false;
+// warp-uniform; `primary_done` is this warp's sticky note that the primary source is exhausted (the cursor only grows),
+// which in k-mode (no secondaries) makes every later call free of global loads
+__device__ __forceinline__ bool source_has_work(const DevRun &R, bool &primary_done) {
+  if (primary_done && R.kmode) return false;
+  int yes = 0;
   if ((threadIdx.x & 31) == 0) {
-    yes = ld_vol(R.src_next) < R.src_total;
-    if (!yes && !R.kmode) yes = ld_vol(R.sec_head) < ld_vol(R.sec_tail);
+    if (!primary_done) yes = ld_vol(R.src_next) < R.src_total ? 1 : 2;
+    if (yes != 1 && !R.kmode && ld_vol(R.sec_head) < ld_vol(R.sec_tail)) yes |= 1;
   }
-  return __shfl_sync(FULL, (int)yes, 0) != 0;
+  yes = __shfl_sync(FULL, yes, 0);
+  if (yes & 2) primary_done = true;
+  return (yes & 1) != 0;
 }
 
 // ---------------------------------------------------------------------------------- the persistent kernel
@@ -260,7 +265,7 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R) {       // warp
 #define TDR_ASYNC_MINB 2
 #endif
 template <bool CE, int MODE>
-__global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max) {
+__global__ void __launch_bounds__(512, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -276,15 +281,24 @@ __global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut
   const int first_ev = SPLIT ? EV_LOOKUP : EV_STEP;
   i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
   u32 myfree = NOSLOT;                        // a slot this lane owns that holds no particle
-  bool starved = false;
+  bool starved = false, primary_done = false;
   u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
+  bool done = false;
   for (;;) {
+    // Lockstep: the warps of a CTA pass the loop top together, so that they run the same event code at the same time
+    // and an instruction line fetched for one warp serves the others from the SM's instruction cache (the loop is
+    // instruction-fetch bound, profiles/ncu_r01.md).  A warp with nothing to do keeps voting (and keeps looking for
+    // work) until every warp of its CTA is done; the CTA then leaves as one.  Only warps of the SAME CTA meet at
+    // this barrier, and each arrives after a bounded amount of its own work: no warp waits for another CTA.
+    if (lockstep) { if (__syncthreads_and(done ? 1 : 0)) break; done = false; }
     int l = -1, fi = -1;
     if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
     else {
-      if (source_has_work(R)) {
+      // make_work by a starved warp: only a warp that may still grow its pool of slots, or that holds
+      // spare ones, asks; the others are refilled through their SOURCE links
+      if ((fresh < fresh_max || __any_sync(FULL, myfree != NOSLOT)) && source_has_work(R, primary_done)) {
         // starved warp: every lane brings a slot (its own spare one, else a fresh one from the window) and claims work
         u32 need = __ballot_sync(FULL, myfree == NOSLOT);
         if (fresh >= fresh_max) need = 0;                       // this warp's pool of slots is large enough
@@ -302,8 +316,12 @@ __global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut
         n_makework++;
         if (__any_sync(FULL, born)) { stash_insert(w, first_ev, slot, born); if (s.nfull() > 0) continue; }
       }
-      int bc = 0;
-      for (int e = 0; e < EV_COUNT; e++) { int pl = s.partial(e); if (pl >= 0 && s.cnt(pl) > bc) { l = pl; bc = s.cnt(pl); } }
+      int bc = 0;                                                 // fullest partial link among this mode's event types
+      constexpr int n_ev = MODE == 0 ? 2 : MODE == 2 ? 3 : 6;
+      constexpr int evs[3][6] = { { EV_STEP, EV_SOURCE, 0, 0, 0, 0 }, { EV_LOOKUP, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_SOURCE },
+                                  { EV_STEP, EV_COLLIDE, EV_SOURCE, 0, 0, 0 } };
+#pragma unroll
+      for (int k = 0; k < n_ev; k++) { const int pl = s.partial(evs[MODE][k]); const int pc = pl >= 0 ? s.cnt(pl) : 0; if (pc > bc) { l = pl; bc = pc; } }
       if (l < 0) {
         if (fetch_link(w)) continue;
         // nothing anywhere in reach: publish what this warp knows, then leave or wait (no other warp is waited for)
@@ -315,9 +333,10 @@ __global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut
           else if (starved && global_ns() - t_idle > deadline_ns) { atomicExch(O.err, TDR_ELOST); er = 1; }
         }
         out = __shfl_sync(FULL, out, 0); er = __shfl_sync(FULL, er, 0);
-        if (out == 0 || er != 0) break;
+        if (out == 0 || er != 0) { if (!lockstep) break; done = true; continue; }
         if (!starved) { starved = true; if (w.lane == 0) { atomicAdd(R.starved, 1ull); t_idle = global_ns(); } }
-        __nanosleep(backoff); if (backoff < 8000) backoff += backoff;      // idle warps leave the issue slots to the others
+        if (lockstep) __nanosleep(400);                               // the CTA's busy warps wait for this one at the barrier
+        else { __nanosleep(backoff); if (backoff < 8000) backoff += backoff; }   // idle warps leave the issue slots to the others
         continue;
       }
     }
@@ -329,7 +348,7 @@ __global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut
         A.actr[AC_DBG] = w.gw; A.actr[AC_DBG + 1] = (u64)s.cnt(l); A.actr[AC_DBG + 2] = (u64)s.ev(l); A.actr[AC_DBG + 3] = (u64)s.nfull();
         A.actr[AC_DBG + 4] = (u64)s.nfree(); A.actr[AC_DBG + 5] = n_iter; A.actr[AC_DBG + 6] = n_events; A.actr[AC_DBG + 7] = (u64)delta;
       }
-      if (__shfl_sync(FULL, ex, 0)) break;
+      if (__shfl_sync(FULL, ex, 0) && !lockstep) break;           // in lockstep the CTA leaves as one, once every warp sees the error
     }
     // take the link out of the stash, then run its event on all lanes
     const int c = s.cnt(l), e = s.ev(l);
@@ -349,7 +368,7 @@ __global__ void __launch_bounds__(256, TDR_ASYNC_MINB) k_async(DevProb P, DevOut
       if (valid) { id = S.id[slot]; sg = S.seg[slot]; nc = S.ncoll[slot]; }
       record_deaths_warp(&acc, R, valid, id, sg, nc);
       bool born = false;
-      if (source_has_work(R)) { born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, valid); n_makework++; }
+      if (source_has_work(R, primary_done)) { born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, valid); n_makework++; }
       if (born) store_part<CE>(S, slot, p);
       else if (valid && myfree == NOSLOT) myfree = slot;
       stash_insert(w, first_ev, slot, born);
