@@ -171,8 +171,8 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
-  else if (k == "lockstep") p->lockstep = atoi(value) != 0;
-  else if (k == "async_threads") { int n = atoi(value); if (n != 128 && n != 256 && n != 512) return fail(TDR_EINVAL, "async_threads in {128,256,512}"); p->async_threads = n; }
+  else if (k == "lockstep") { int n = atoi(value); if (n < 0 || n > 64) return fail(TDR_EINVAL, "lockstep in [0,64]"); p->lockstep = n; }
+  else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > 1024 || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,1024]"); p->async_threads = n; }
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
@@ -395,7 +395,7 @@ static int run_async(tdr_problem *p, DevRun R) {
   const size_t smem = smem_bytes(p) + (threads / 32) * (size_t)STASH_WORDS(p->stash_links) * 4;
   R.defer_death = 1; R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
-  k_async_init<<<1, 64, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
+  k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
   LAUNCH_CHECK();
   if (p->split == 1) launch_async<CE, 1>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2>(p, R, smem, threads); else launch_async<CE, 0>(p, R, smem, threads);
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;

@@ -73,17 +73,19 @@ __device__ __noinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) 
   return NOLINK;
 }
 
-// builds the empty-link queues (arena link i belongs to queue i % AQ) and resets the scheduler counters
+// builds the empty-link queues (arena link i belongs to queue i % AQ, chained in index order) and resets the
+// scheduler counters; any grid
 __global__ void k_async_init(AsyncMem A, u64 *outstanding, u64 n_source, u64 *slot_next, u64 *starved) {
-  u32 q = threadIdx.x;
-  if (q < AQ) {
-    u32 last = NOLINK, first = NOLINK;
-    for (u64 i = q; i < A.n_links; i += AQ) { if (first == NOLINK) first = (u32)i; A.links[i].next = (i + AQ < A.n_links) ? (u32)(i + AQ) : NOLINK; last = (u32)i; }
-    A.q_empty[q] = first == NOLINK ? NULLQ : (((u64)first << 32) | last);
+  const u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x, nt = (u64)gridDim.x * blockDim.x;
+  for (u64 i = t; i < A.n_links; i += nt) A.links[i].next = (i + AQ < A.n_links) ? (u32)(i + AQ) : NOLINK;
+  if (t < AQ) {
+    const u64 q = t;
+    u64 last = A.n_links > q ? q + ((A.n_links - 1 - q) / AQ) * AQ : 0;
+    A.q_empty[q] = A.n_links > q ? ((q << 32) | last) : NULLQ;
     A.q_work[q] = NULLQ;
   }
-  if (q < AC_COUNT) A.actr[q] = 0;
-  if (q == 0) { *outstanding = n_source; *slot_next = 0; *starved = 0; }
+  if (t < AC_COUNT) A.actr[t] = 0;
+  if (t == 0) { *outstanding = n_source; *slot_next = 0; *starved = 0; }
 }
 
 // ---------------------------------------------------------------------------------- stash (per warp, shared memory)
@@ -265,7 +267,10 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R, bool &primary_d
 #define TDR_ASYNC_MINB 2
 #endif
 template <bool CE, int MODE>
-__global__ void __launch_bounds__(512, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep) {
+#ifndef TDR_ASYNC_MAXT
+#define TDR_ASYNC_MAXT 512
+#endif
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -285,14 +290,14 @@ __global__ void __launch_bounds__(512, 1) k_async(DevProb P, DevOut O, DevRun R,
   u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
-  bool done = false;
+  bool done = false; u32 n_pass = 0;
   for (;;) {
     // Lockstep: the warps of a CTA pass the loop top together, so that they run the same event code at the same time
     // and an instruction line fetched for one warp serves the others from the SM's instruction cache (the loop is
     // instruction-fetch bound, profiles/ncu_r01.md).  A warp with nothing to do keeps voting (and keeps looking for
     // work) until every warp of its CTA is done; the CTA then leaves as one.  Only warps of the SAME CTA meet at
     // this barrier, and each arrives after a bounded amount of its own work: no warp waits for another CTA.
-    if (lockstep) { if (__syncthreads_and(done ? 1 : 0)) break; done = false; }
+    if (lockstep && (++n_pass % (u32)lockstep) == 0) { if (__syncthreads_and(done ? 1 : 0)) break; done = false; }
     int l = -1, fi = -1;
     if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
     else {

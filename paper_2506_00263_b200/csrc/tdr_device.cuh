@@ -75,7 +75,7 @@ struct Part {
 // ---------------------------------------------------------------------------------- R1 Philox4x32-10
 struct Blk { u32 w0, w1, w2, w3; };
 
-__device__ __noinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {      // one copy in the instruction cache
+__device__ __forceinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {
 #pragma unroll
   for (int r = 0; r < 10; r++) {
     u32 h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;

@@ -141,6 +141,7 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
   const u64 n_in = *count_in;
   i64 accP = 0, accPc = 0;
   for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_in; i0 += (u64)gridDim.x * blockDim.x) {
+    __syncthreads();       // the CTA's warps start each tile together: they share the instruction lines they fetch
     u64 i = i0 + threadIdx.x;
     bool valid = i < n_in;
     Part p; u32 slot = 0;
