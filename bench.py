@@ -136,7 +136,23 @@ def cpu_baseline():
     segs = r["totals"]["n_seg"]
     return {"value": segs / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"cfg1 at {n} particles/gen, {gi}+{ga} generations ({segs} segments, {dt:.1f} s)",
-            "histories_per_sec": float(r["gen_n"].sum()) / dt}
+            "histories_per_sec": float(r["gen_n"].sum()) / dt}, r, (n, gi, ga)
+
+
+def full_size_parity(o, kept):
+    """The oracle's run of the full workload against every timed CUDA variant: totals (incl. the order-independent
+    per-history digest), int64 tallies, leak, per-generation N/M/P/Pc bit-exact; k to 1e-12."""
+    import numpy as np
+    bad = []
+    for name, g in kept.items():
+        ok = o["totals"] == g["totals"]
+        for k in ("flux", "coll", "leak", "gen_n", "gen_m", "gen_p", "gen_pc"):
+            ok = ok and np.array_equal(o[k], g[k])
+        ok = ok and np.allclose(o["gen_k"], g["gen_k"], rtol=1e-12, atol=0) and abs(o["k_mean"] - g["k_mean"]) <= 1e-12 * abs(o["k_mean"])
+        if not ok:
+            bad.append(name)
+    return {"checked": "full workload vs oracle: totals + history digest, flux, coll, leak, per-generation N/M/P/Pc (bit-exact), k (1e-12)",
+            "variants": sorted(kept), "ok": not bad, "mismatch": bad}
 
 
 def run_ours(args, rank, world, local_rank):
@@ -156,7 +172,7 @@ def run_ours(args, rank, world, local_rank):
             dist.barrier()
         torch.cuda.synchronize()
 
-    results = {}
+    results, kept = {}, {}
     if args.scheme == "all":
         variants = [("async", "hybrid"), ("async", "fused"), ("stack", "fused"), ("stack", "hybrid")]
     else:
@@ -183,6 +199,7 @@ def run_ours(args, rank, world, local_rank):
         ms = e0.elapsed_time(e1)
         clocks = sampler.stop() if sampler else None
         res = P.read_tallies(history=False, bank=False)
+        kept[f"{scheme}/{decomp}"] = res
         seg_step, hist_step = res["totals"]["n_seg"], int(res["gen_n"].sum())      # identical every step (same seed)
         segs, hist = seg_step * args.steps, hist_step * args.steps
         P.close()
@@ -239,7 +256,11 @@ def run_ours(args, rank, world, local_rank):
                 "clocks": first["clocks"], "roofline": first["roofline"], "roofline_issue": first["roofline_issue"],
                 "schemes": {k: {kk: vv for kk, vv in v.items() if kk != "clocks"} for k, v in results.items()}}
         if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_baseline()
+            line["cpu_baseline"], o_res, o_cfg = cpu_baseline()
+            if o_cfg == (n, gi, ga):
+                line["parity_full_size"] = full_size_parity(o_res, kept)
+                if not line["parity_full_size"]["ok"]:
+                    print(json.dumps(line)); raise SystemExit("full-size parity FAILED: " + str(line["parity_full_size"]["mismatch"]))
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -247,12 +247,13 @@ static int grid_for(tdr_problem *p, K kernel, size_t smem, int threads = 256) {
 
 struct KTimer {                                   // optional CUDA-event bracket around the dominant kernel's launches
   tdr_problem *p; bool on;
-  KTimer(tdr_problem *p_, bool dominant) : p(p_), on(p_->time_kernels && dominant) {
+  int n;                                          // launches inside the bracket (they run back to back on the stream)
+  KTimer(tdr_problem *p_, bool dominant, int n_ = 1) : p(p_), on(p_->time_kernels && dominant), n(n_) {
     if (!on) return;
     while (p->ev_pool.size() < p->ev_used + 2) { cudaEvent_t e; cudaEventCreate(&e); p->ev_pool.push_back(e); }
     cudaEventRecord(p->ev_pool[p->ev_used], p->stream);
   }
-  ~KTimer() { if (on) { cudaEventRecord(p->ev_pool[p->ev_used + 1], p->stream); p->ev_used += 2; p->diag.step_launches++; } }
+  ~KTimer() { if (on) { cudaEventRecord(p->ev_pool[p->ev_used + 1], p->stream); p->ev_used += 2; p->diag.step_launches += n; } }
 };
 
 static void collect_kernel_times(tdr_problem *p) {
@@ -334,12 +335,13 @@ static int run_stack(tdr_problem *p, DevRun R) {
     const int batch = n_in * 4 > W ? 1 : p->sync_every;
     u64 blocks64 = (n_in + 255) / 256; int cap_blocks = blocks64 > (1u << 30) ? (1 << 30) : (int)blocks64;
     if (cap_blocks < 1) cap_blocks = 1;
+    {
+    KTimer tb(p, !split, batch * (hybrid ? 2 : 1));     // one event pair per batch: the launches run back to back
     for (int b = 0; b < batch; b++) {
       if (!split) {
         const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
         u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // hybrid: collide-stack counters
         const int g1 = g_step < cap_blocks ? g_step : cap_blocks;
-        KTimer t(p, true);
         if (hybrid) {
           k_step<CE, true><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
                                                   p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz);
@@ -352,6 +354,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
         LAUNCH_CHECK(); p->diag.kernel_launches++;
       } else if ((rc = split_iteration<CE>(p, R, smem, sg, cap_blocks))) return rc;
       it++; p->diag.iterations++;
+    }
     }
     CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));

@@ -105,3 +105,13 @@ def test_fixed_source_sharded_by_id_ranges_sums_to_the_full_run(scheme):
         for k in ("flux", "coll", "leak"):
             assert np.array_equal(m[k], o[k]), (p.name, k)
         assert m["totals"] == o["totals"], p.name
+
+
+@pytest.mark.parametrize("scheme,decomp", [("async", "fused"), ("stack", "fused")])
+def test_full_size_cfg1_and_cfg3_match_the_oracle(scheme, decomp):
+    """BASELINE.json's full sizes, in the launch configuration bench.py times: cfg1 at 1e6 particles/generation
+    (10 of the 70 generations, to bound the oracle's time) and cfg3 at 1e6 histories.  Everything that is unique is
+    compared: totals with the order-independent per-history digest, all tallies, per-generation sums, the bank."""
+    for p in (W.cfg1(n_inactive=3, n_active=7), W.cfg3(n=1000000, n_ebins=100)):
+        o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+        assert_same(o, g, f"full-size {p.name}/{scheme}")
