@@ -35,7 +35,8 @@ struct tdr_problem {
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
-  int sync_every = 8;                      // stack scheme: remap iterations launched per counter read-back
+  int drain_below = 65536;                 // stack scheme, k-mode: population below which the tail is drained in one launch
+  int sync_every = 16;                      // stack scheme: remap iterations launched per counter read-back
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
   // carved pointers (valid during/after a run)
@@ -176,6 +177,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
+  else if (k == "drain_below") { int n = atoi(value); if (n < 0) return fail(TDR_EINVAL, "drain_below >= 0"); p->drain_below = n; }
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -365,6 +367,19 @@ static int run_stack(tdr_problem *p, DevRun R) {
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
     h_sec_head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;          // claims past the limit got nothing
     const u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
+    if (!split && R.kmode && rem == 0 && alive > 0 && alive <= (u64)p->drain_below) {
+      // tail drain: the few particles left are followed to their death in ONE launch (k_drain)
+      const int blocks = (int)((alive + 63) / 64);
+      {
+        KTimer td(p, true);
+        k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + it % 3);
+      }
+      LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.iterations++;
+      CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+      CK(cudaStreamSynchronize(st));
+      if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
+      break;
+    }
     if (alive == 0) {
       if (pend + rem == 0) break;
       u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;

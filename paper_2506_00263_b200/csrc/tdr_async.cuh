@@ -297,7 +297,12 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
     // instruction-fetch bound, profiles/ncu_r01.md).  A warp with nothing to do keeps voting (and keeps looking for
     // work) until every warp of its CTA is done; the CTA then leaves as one.  Only warps of the SAME CTA meet at
     // this barrier, and each arrives after a bounded amount of its own work: no warp waits for another CTA.
-    if (lockstep && (++n_pass % (u32)lockstep) == 0) { if (__syncthreads_and(done ? 1 : 0)) break; done = false; }
+    if (lockstep && (++n_pass % (u32)lockstep) == 0) {
+      // the vote: every warp is done, or (k-mode) has seen the source exhausted -> the CTA drops the lockstep for the
+      // tail; a warp that is done then leaves on its own, the others drain their links without a barrier
+      if (__syncthreads_and((done || (MODE == 0 && R.kmode && primary_done)) ? 1 : 0)) lockstep = 0;
+      done = false;
+    }
     int l = -1, fi = -1;
     if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
     else {
@@ -380,6 +385,24 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       continue;
     }
     n_events += (u32)c;
+    if (MODE == 0 && !lockstep && R.kmode && primary_done && fi < 0) {     // fi < 0: the warp's last (partial) STEP link
+      // Tail of a generation (source exhausted, lockstep dropped, fewer than 32 particles left in this warp): nothing is
+      // left to regroup with, so the link's particles are followed to their death in registers instead of going through L2 and the stash after every
+      // segment (the monolithic scheme is "history-length truncation with length 1"; the length is
+      // unbounded once remapping has no fresh work to merge in).  Deaths still go through the SOURCE link.
+      if (valid) load_part<CE>(S, slot, p);
+      bool live = valid;
+      while (__any_sync(FULL, live)) {
+        int nc1 = 0, cs1 = 0;
+        const int nx = exec_event<CE, EV_STEP, false, 0>(P, mg, O, tp, R, S, &acc, slot, live, p, nc1, cs1, accP, accPc, first_ev);
+        if (__any_sync(FULL, nc1 > 0)) push_children(O, R, &acc, p, nc1, cs1);
+        if (live && nx == NEXT_DEAD) live = false;
+        n_events += (u32)__popc(__ballot_sync(FULL, live));
+      }
+      delta -= (i64)c;
+      stash_insert(w, EV_SOURCE, slot, valid);
+      continue;
+    }
     if (MODE == 0) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
     else if (MODE == 2) {
       if (e == EV_STEP) next = exec_event<CE, EV_STEP, true>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);

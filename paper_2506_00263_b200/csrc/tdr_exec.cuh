@@ -15,7 +15,8 @@ __device__ __forceinline__ void load_loc_energy(const Soa &S, u32 i, Part &p) {
 }
 
 // returns the next event of this lane's particle (NEXT_DEAD if it died or the lane is idle)
-template <bool CE, int EV, bool HYBRID = false>
+// IO (EV_STEP only): bit 0 = load the particle from the SoA state first, bit 1 = store a survivor back
+template <bool CE, int EV, bool HYBRID = false, int IO = 3>
 __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, const DevOut &O, const TallyPriv &tp, const DevRun &R, const Soa &S,
                                           BlockAcc *acc, u32 slot, bool valid, Part &p, int &nch, int &csrc,
                                           i64 &accP, i64 &accPc, int first_ev) {
@@ -23,7 +24,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
   if (EV == EV_STEP) {                                   // monolithic step: T1..T8 in one event
     double St = 0.0, nsf = 0.0, d = 0.0, f = 0.0; int gi = 0; u32 flags = 0;
     if (valid) {
-      load_part<CE>(S, slot, p);
+      if (IO & 1) load_part<CE>(S, slot, p);
       ev_lookup<CE>(P, mg, p, St, nsf, gi, f);
       ev_move(P, R.seed, R.gen, p, St, d, flags);
     }
@@ -40,7 +41,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
         alive = ev_collide<CE>(P, mg, R, acc, p, St, gi, f, nch, csrc);
       }
       else alive = ev_surface(P, R, acc, p, flags);
-      if (alive) store_part<CE>(S, slot, p);
+      if (alive) { if (IO & 2) store_part<CE>(S, slot, p); }
       else if (R.defer_death) { S.seg[slot] = p.seg; S.ncoll[slot] = p.ncoll; }
     }
     return alive ? EV_STEP : NEXT_DEAD;

@@ -175,6 +175,43 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
   priv_flush(tp, O);
 }
 
+// ---------------------------------------------------------------------------------- tail drain (stack scheme, k-mode)
+// Once the source is exhausted and only a few thousand particles are left, a remap iteration is a kernel launch
+// that lasts one segment's latency (the "fixed costs" of PAPER.md:153).  This kernel pops the step stack once and
+// follows each remaining particle to its death in registers: one launch instead of ~100.  No make_work (nothing is
+// left to claim), children go to the fission bank as usual; a warp keeps calling the warp-cooperative tally until
+// its last lane is done.
+template <bool CE>
+__global__ void __launch_bounds__(256) k_drain(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in) {
+  extern __shared__ double smem[];
+  __shared__ BlockAcc acc;
+  const double *mg = stage_mg(P, smem);
+  const TallyPriv tp = stage_priv(P, smem);
+  acc_init(&acc);
+  const u64 n_in = *count_in;
+  i64 accP = 0, accPc = 0;
+  for (u64 i0 = (u64)blockIdx.x * blockDim.x; i0 < n_in; i0 += (u64)gridDim.x * blockDim.x) {
+    const u64 i = i0 + threadIdx.x;
+    bool live = i < n_in;
+    Part p;
+    if (live) load_part<CE>(S, stack_in[i], p);
+    while (__any_sync(FULL, live)) {
+      double St = 0.0, nsf = 0.0, d = 0.0, f = 0.0; int gi = 0; u32 flags = 0;
+      if (live) { ev_lookup<CE>(P, mg, p, St, nsf, gi, f); ev_move(P, R.seed, R.gen, p, St, d, flags); }
+      ev_tally<CE>(P, O, tp, R, p, live && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
+      int nch = 0, csrc = 0;
+      if (live) {
+        if ((flags & F_LOST) || p.seg >= (1u << 24)) { atomicExch(O.err, TDR_ELOST); live = false; }
+        else if (flags & F_COLLIDE) live = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+        else live = ev_surface(P, R, &acc, p, flags);
+      }
+      push_children(O, R, &acc, p, nch, csrc);
+    }
+  }
+  acc_flush(&acc, O, accP, accPc);
+  priv_flush(tp, O);
+}
+
 // ---------------------------------------------------------------------------------- A9 population control (D2)
 __global__ void __launch_bounds__(256) k_popctrl(const tdr_site *bank, u64 n_bank, tdr_site *next, u64 next_cap, u64 *next_count,
                                                  u64 seed, u32 gen_next, double pr, int *err) {
