@@ -32,6 +32,7 @@ struct tdr_problem {
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
   int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
+  int seg_per_event = 2;                   // async fused: segments a particle is followed per step event before remapping
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
@@ -174,6 +175,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "time_kernels") p->time_kernels = atoi(value);
   else if (k == "lockstep") { int n = atoi(value); if (n < 0 || n > 64) return fail(TDR_EINVAL, "lockstep in [0,64]"); p->lockstep = n; }
   else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > 1024 || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,1024]"); p->async_threads = n; }
+  else if (k == "seg_per_event") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "seg_per_event in [1,1024]"); p->seg_per_event = n; }
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
@@ -402,7 +404,7 @@ static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int thread
   int grid = grid_for(p, k_async<CE, MODE>, smem, threads);
   KTimer t(p, true);
   k_async<CE, MODE><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
-                                                        (u32)p->slots_per_warp, p->lockstep);
+                                                        (u32)p->slots_per_warp, p->lockstep, (u32)p->seg_per_event);
   return 0;
 }
 

@@ -270,7 +270,7 @@ template <bool CE, int MODE>
 #ifndef TDR_ASYNC_MAXT
 #define TDR_ASYNC_MAXT 512
 #endif
-__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep) {
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -385,26 +385,35 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       continue;
     }
     n_events += (u32)c;
-    if (MODE == 0 && !lockstep && R.kmode && primary_done && fi < 0) {     // fi < 0: the warp's last (partial) STEP link
-      // Tail of a generation (source exhausted, lockstep dropped, fewer than 32 particles left in this warp): nothing is
-      // left to regroup with, so the link's particles are followed to their death in registers instead of going through L2 and the stash after every
-      // segment (the monolithic scheme is "history-length truncation with length 1"; the length is
-      // unbounded once remapping has no fresh work to merge in).  Deaths still go through the SOURCE link.
+    if (MODE == 0) {
+      // Monolithic scheme: the `step` event is "history-length truncation with length 1".  Here the
+      // length is seg_per_event: a particle is followed for up to that many segments in registers before it goes
+      // back through L2 and the stash to be regrouped; a lane whose particle dies idles until the event ends.  In the
+      // tail of a generation (k-mode, source exhausted, lockstep dropped, the warp's last partial link) nothing is left
+      // to regroup with and the length is unbounded.  Deaths go through the SOURCE link either way.
+      const u32 kmax = (!lockstep && R.kmode && primary_done && fi < 0) ? 0xFFFFFFFFu : seg_per_event;
       if (valid) load_part<CE>(S, slot, p);
-      bool live = valid;
-      while (__any_sync(FULL, live)) {
+      bool live = valid; u32 nc_tot = 0;
+      for (u32 k = 0; k < kmax; k++) {
         int nc1 = 0, cs1 = 0;
         const int nx = exec_event<CE, EV_STEP, false, 0>(P, mg, O, tp, R, S, &acc, slot, live, p, nc1, cs1, accP, accPc, first_ev);
-        if (__any_sync(FULL, nc1 > 0)) push_children(O, R, &acc, p, nc1, cs1);
+        const u32 ncw = __reduce_add_sync(FULL, (u32)nc1);
+        if (ncw) { push_children(O, R, &acc, p, nc1, cs1); nc_tot += ncw; }
         if (live && nx == NEXT_DEAD) live = false;
-        n_events += (u32)__popc(__ballot_sync(FULL, live));
+        const u32 lm = __ballot_sync(FULL, live);
+        if (lm == 0) break;
+        if (k + 1 < kmax) n_events += (u32)__popc(lm);
       }
-      delta -= (i64)c;
-      stash_insert(w, EV_SOURCE, slot, valid);
+      if (live) store_part<CE>(S, slot, p);
+      const bool died = valid && !live;
+      const u32 dm = __ballot_sync(FULL, died);
+      delta += (R.kmode ? 0 : (i64)nc_tot) - (i64)__popc(dm);
+      if (dm) stash_insert(w, EV_SOURCE, slot, died);
+      stash_insert(w, EV_STEP, slot, live);
+      if ((++n_iter & 63u) == 0 && delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
       continue;
     }
-    if (MODE == 0) next = exec_event<CE, EV_STEP>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
-    else if (MODE == 2) {
+    if (MODE == 2) {
       if (e == EV_STEP) next = exec_event<CE, EV_STEP, true>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
       else next = exec_event<CE, EV_COLLIDE>(P, mg, O, tp, R, S, &acc, slot, valid, p, nch, csrc, accP, accPc, first_ev);
     }
@@ -423,8 +432,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       delta += (R.kmode ? 0 : (i64)nc) - (i64)__popc(dm);     // k-mode children belong to the next generation
       stash_insert(w, EV_SOURCE, slot, died);                   // the slot waits for the SOURCE event
     }
-    if (MODE == 0) stash_insert(w, EV_STEP, slot, next == EV_STEP);
-    else if (MODE == 2) { stash_insert(w, EV_STEP, slot, next == EV_STEP); if (e == EV_STEP) stash_insert(w, EV_COLLIDE, slot, next == EV_COLLIDE); }
+    if (MODE == 2) { stash_insert(w, EV_STEP, slot, next == EV_STEP); if (e == EV_STEP) stash_insert(w, EV_COLLIDE, slot, next == EV_COLLIDE); }
     else {
       if (e == EV_LOOKUP) stash_insert(w, EV_MOVE, slot, next == EV_MOVE);
       else if (e == EV_MOVE) stash_insert(w, EV_TALLY, slot, next == EV_TALLY);
