@@ -128,7 +128,7 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
 template <bool CE, bool HYBRID>
 __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in,
                                               u32 *stack_out, u64 *count_out, u64 *count_zero,
-                                              u32 *cstack, u64 *ccount, u64 *ccount_zero) {
+                                              u32 *cstack, u64 *ccount, u64 *ccount_zero, u32 seg_per_launch) {
   if (blockIdx.x == 0 && threadIdx.x == 0) {       // the stacks the previous launches drained (rotating counters)
     *count_zero = 0;
     if (HYBRID) *ccount_zero = 0;
@@ -145,27 +145,31 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
     u64 i = i0 + threadIdx.x;
     bool valid = i < n_in;
     Part p; u32 slot = 0;
-    double St = 0.0, nsf = 0.0, d = 0.0, f = 0.0; int gi = 0; u32 flags = 0;
-    if (valid) {
-      slot = stack_in[i];
-      load_part<CE>(S, slot, p);
-      ev_lookup<CE>(P, mg, p, St, nsf, gi, f);
-      ev_move(P, R.seed, R.gen, p, St, d, flags);
-    }
-    ev_tally<CE>(P, O, tp, R, p, valid && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
-    bool alive = false, to_collide = false; int nch = 0, csrc = 0;
-    if (valid) {
-      if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
-      else if (flags & F_COLLIDE) {
-        if (HYBRID) {
-          S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; S.s_sigt[slot] = St;
-          if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
-          to_collide = true;
-        } else alive = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+    if (valid) { slot = stack_in[i]; load_part<CE>(S, slot, p); }
+    // up to seg_per_launch segments per particle in registers before it is pushed again ("history-length truncation",
+    // PAPER.md:119, with a length > 1): fewer launches and state round trips; a lane whose particle died idles
+    bool alive = valid, to_collide = false;
+    for (u32 k = 0; k < seg_per_launch; k++) {
+      double St = 0.0, nsf = 0.0, d = 0.0, f = 0.0; int gi = 0; u32 flags = 0;
+      if (alive) { ev_lookup<CE>(P, mg, p, St, nsf, gi, f); ev_move(P, R.seed, R.gen, p, St, d, flags); }
+      ev_tally<CE>(P, O, tp, R, p, alive && !(flags & F_LOST), d, St, nsf, flags, accP, accPc);
+      int nch = 0, csrc = 0;
+      if (alive) {
+        if ((flags & F_LOST) || p.seg >= (1u << 24)) { atomicExch(O.err, TDR_ELOST); alive = false; }
+        else if (flags & F_COLLIDE) {
+          if (HYBRID) {
+            if (k > 0) store_part<CE>(S, slot, p);       // an earlier crossing of this launch changed direction / indices too
+            else { S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; }
+            S.s_sigt[slot] = St;
+            if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
+            to_collide = true; alive = false;
+          } else alive = ev_collide<CE>(P, mg, R, &acc, p, St, gi, f, nch, csrc);
+        }
+        else alive = ev_surface(P, R, &acc, p, flags);
       }
-      else alive = ev_surface(P, R, &acc, p, flags);
+      if (!HYBRID) push_children(O, R, &acc, p, nch, csrc);
+      if (!__any_sync(FULL, alive)) break;
     }
-    if (!HYBRID) push_children(O, R, &acc, p, nch, csrc);
     if (make_work<CE>(P, mg, R, &acc, p, valid && !alive && !to_collide)) alive = true;
     if (alive) store_part<CE>(S, slot, p);
     stack_push(stack_out, count_out, slot, alive);
