@@ -38,7 +38,7 @@ struct tdr_problem {
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
   int drain_below = 65536;                 // stack scheme, k-mode: population below which the tail is drained in one launch
-  int sync_every = 16;                      // stack scheme: remap iterations launched per counter read-back
+  int sync_every = 6;                      // stack scheme: remap iterations launched per counter read-back
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
   // carved pointers (valid during/after a run)
