@@ -121,7 +121,8 @@ int tdr_init_problem(const tdr_geometry *, const tdr_materials *, const tdr_xs_t
 /* keys: "scheme" = stack|async; "decomposition" = fused|split|hybrid; "window" = particles in flight;
  * "stash_links" (async, links per warp, 8..64); "slots_per_warp" (async); "sync_every" (stack: remap iterations per
  * counter read-back); "blocks_per_sm"; "keep_history" = 0|1; "time_kernels" = 0|1; "idle_timeout_s" (async watchdog);
- * "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs).
+ * "seg_per_event" (async fused: segments per step event); "seg_per_launch", "drain_below" (stack); "lockstep",
+ * "async_threads" (async); "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs).
  * decomposition = fused (monolithic step) | split (five events) | hybrid (step + collide). */
 int tdr_set_option(tdr_problem *, const char *key, const char *value);
 int tdr_workspace_bytes(const tdr_problem *, uint64_t n_particles, uint64_t *bytes);
