@@ -290,14 +290,18 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
   u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
-  bool done = false; u32 n_pass = 0;
+  bool done = false; u32 inner_used = 0;
   for (;;) {
     // Lockstep: the warps of a CTA pass the loop top together, so that they run the same event code at the same time
     // and an instruction line fetched for one warp serves the others from the SM's instruction cache (the loop is
     // instruction-fetch bound, profiles/ncu_r01.md).  A warp with nothing to do keeps voting (and keeps looking for
     // work) until every warp of its CTA is done; the CTA then leaves as one.  Only warps of the SAME CTA meet at
     // this barrier, and each arrives after a bounded amount of its own work: no warp waits for another CTA.
-    if (lockstep && (++n_pass % (u32)lockstep) == 0) {
+    if (lockstep) {
+      // Between two votes every warp of the CTA passes exactly seg_per_event - 1 further barriers: a step event meets
+      // them between its segments (so the segments of all warps start together as well), every other path makes up
+      // for them here.
+      if (MODE == 0) { for (u32 j = inner_used; j + 1 < seg_per_event; j++) __syncthreads_and(1); inner_used = 0; }
       // the vote: every warp is done, or (k-mode) has seen the source exhausted -> the CTA drops the lockstep for the
       // tail; a warp that is done then leaves on its own, the others drain their links without a barrier
       if (__syncthreads_and((done || (MODE == 0 && R.kmode && primary_done)) ? 1 : 0)) lockstep = 0;
@@ -402,7 +406,10 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
         if (live && nx == NEXT_DEAD) live = false;
         const u32 lm = __ballot_sync(FULL, live);
         if (lm == 0) break;
-        if (k + 1 < kmax) n_events += (u32)__popc(lm);
+        if (k + 1 < kmax) {
+          n_events += (u32)__popc(lm);
+          if (lockstep) { __syncthreads_and(1); inner_used++; }
+        }
       }
       if (live) store_part<CE>(S, slot, p);
       const bool died = valid && !live;

@@ -199,7 +199,9 @@ __device__ __forceinline__ double plane_dist(double lo, double hi, double x, dou
   // an infinite plane or a zero direction component gives +inf (G3) without entering the division: infinite or
   // zero operands would send the whole warp through the slow path of the software fp64 division
   const bool ok = (c != 0.0) && (fabs(num) < TDR_INF);
-  const double d = (ok ? num : 1.0) / (ok ? c : 1.0);
+  double ns = ok ? num : 1.0, cs = ok ? c : 1.0;
+  asm volatile("" : "+d"(ns), "+d"(cs));   // opaque: otherwise the compiler sees the result unused and divides inf by c anyway
+  const double d = ns / cs;
   return ok ? d : TDR_INF;
 }
 
@@ -208,7 +210,9 @@ __device__ __forceinline__ double dist_cyl(double X, double Y, double u, double 
   const double b = X * u + Y * v;
   const double c = (X * X + Y * Y) - R * R;
   const double disc = b * b - a * c;
-  const double sq = sqrt(disc < 0.0 ? 0.0 : disc);
+  double dsafe = disc > 0.0 ? disc : 1.0;             // sqrt(0) takes the square root's slow path: a non-positive
+  asm volatile("" : "+d"(dsafe));                     // discriminant gives 0 without entering it
+  const double sq = disc > 0.0 ? sqrt(dsafe) : 0.0;
   double d = (-b + (inside ? sq : -sq)) / a;          // x - y is x + (-y) exactly
   if (d < 0.0) d = 0.0;
   if (!inside && (b >= 0.0 || disc <= 0.0)) d = TDR_INF;
