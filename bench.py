@@ -30,9 +30,9 @@ BYTES_PER_SEGMENT = 150.0
 BYTES_PER_HISTORY = 96.0
 # from the committed ncu captures (profiles/ncu_r01.md): DRAM bytes per launch of the dominant kernel on this workload,
 # and thread-instructions executed per transport segment
-MEASURED_TRAFFIC = {"async/hybrid": 73.3e6, "async/fused": 65.8e6, "stack/fused": 92.2e6}
+MEASURED_TRAFFIC = {"async/hybrid": 73.3e6, "async/fused": 66.1e6, "stack/fused": 92.0e6}
 # stack/fused: k_step runs the same event code as the fused persistent kernel; stack/hybrid: as async/hybrid
-THREAD_INST_PER_SEGMENT = {"async/hybrid": 1473.0, "async/fused": 1134.0, "stack/fused": 1134.0, "stack/hybrid": 1473.0}
+THREAD_INST_PER_SEGMENT = {"async/hybrid": 1473.0, "async/fused": 1046.0, "stack/fused": 1046.0, "stack/hybrid": 1473.0}
 ISSUE_PEAK = 148 * 4 * 32 * 1.965e9
 
 
