@@ -270,7 +270,7 @@ template <bool CE, int MODE>
 #ifndef TDR_ASYNC_MAXT
 #define TDR_ASYNC_MAXT 512
 #endif
-__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event, u32 spill_every) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
   u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
-  bool done = false; u32 inner_used = 0;
+  bool done = false; u32 inner_used = 0, n_top = 0;
   for (;;) {
     // Lockstep: the warps of a CTA pass the loop top together, so that they run the same event code at the same time
     // and an instruction line fetched for one warp serves the others from the SM's instruction cache (the loop is
@@ -307,6 +307,9 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       if (__syncthreads_and((done || (MODE == 0 && R.kmode && primary_done)) ? 1 : 0)) lockstep = 0;
       done = false;
     }
+    // stress option (tests): hand a runnable link to the global queues every spill_every-th pass, so that the spill /
+    // fetch machinery is exercised even when the stash never overflows
+    if (spill_every && s.nfull() > 0 && (++n_top % spill_every) == 0) spill_link(w, s.full(0), 0);
     int l = -1, fi = -1;
     if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
     else {
