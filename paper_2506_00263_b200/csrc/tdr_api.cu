@@ -33,7 +33,7 @@ struct tdr_problem {
   int time_kernels = 0;
   int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
   int seg_per_launch = 3;                  // stack fused/hybrid: segments per particle per k_step launch
-  int spill_every = 0;                     // async stress option: force a spill every n-th scheduler pass (0 = off)
+  int force_spill = 0;                     // async stress option (tests): warps always believe another one is starved
   int seg_per_event = 2;                   // async fused: segments a particle is followed per step event before remapping
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
@@ -178,7 +178,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "lockstep") p->lockstep = atoi(value) != 0;
   else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > 1024 || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,1024]"); p->async_threads = n; }
   else if (k == "seg_per_launch") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "seg_per_launch in [1,1024]"); p->seg_per_launch = n; }
-  else if (k == "spill_every") { int n = atoi(value); if (n < 0 || n == 1) return fail(TDR_EINVAL, "spill_every: 0 (off) or >= 2 (1 would hand every link away for ever)"); p->spill_every = n; }
+  else if (k == "force_spill") p->force_spill = atoi(value) != 0;
   else if (k == "seg_per_event") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "seg_per_event in [1,1024]"); p->seg_per_event = n; }
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
@@ -408,7 +408,7 @@ static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int thread
   int grid = grid_for(p, k_async<CE, MODE>, smem, threads);
   KTimer t(p, true);
   k_async<CE, MODE><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
-                                                        (u32)p->slots_per_warp, p->lockstep, (u32)p->seg_per_event, (u32)p->spill_every);
+                                                        (u32)p->slots_per_warp, p->lockstep, (u32)p->seg_per_event);
   return 0;
 }
 
@@ -419,7 +419,7 @@ static int run_async(tdr_problem *p, DevRun R) {
   const size_t smem = smem_bytes(p) + (threads / 32) * (size_t)STASH_WORDS(p->stash_links) * 4;
   R.defer_death = 1; R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
-  k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved);
+  k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved, p->force_spill ? (1ull << 40) : 0ull);
   LAUNCH_CHECK();
   if (p->split == 1) launch_async<CE, 1>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2>(p, R, smem, threads); else launch_async<CE, 0>(p, R, smem, threads);
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;

@@ -75,7 +75,7 @@ __device__ __noinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) 
 
 // builds the empty-link queues (arena link i belongs to queue i % AQ, chained in index order) and resets the
 // scheduler counters; any grid
-__global__ void k_async_init(AsyncMem A, u64 *outstanding, u64 n_source, u64 *slot_next, u64 *starved) {
+__global__ void k_async_init(AsyncMem A, u64 *outstanding, u64 n_source, u64 *slot_next, u64 *starved, u64 starved0) {
   const u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x, nt = (u64)gridDim.x * blockDim.x;
   for (u64 i = t; i < A.n_links; i += nt) A.links[i].next = (i + AQ < A.n_links) ? (u32)(i + AQ) : NOLINK;
   if (t < AQ) {
@@ -85,7 +85,7 @@ __global__ void k_async_init(AsyncMem A, u64 *outstanding, u64 n_source, u64 *sl
     A.q_work[q] = NULLQ;
   }
   if (t < AC_COUNT) A.actr[t] = 0;
-  if (t == 0) { *outstanding = n_source; *slot_next = 0; *starved = 0; }
+  if (t == 0) { *outstanding = n_source; *slot_next = 0; *starved = starved0; }   // starved0 > 0: stress, every warp believes one is starved
 }
 
 // ---------------------------------------------------------------------------------- stash (per warp, shared memory)
@@ -270,7 +270,7 @@ template <bool CE, int MODE>
 #ifndef TDR_ASYNC_MAXT
 #define TDR_ASYNC_MAXT 512
 #endif
-__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event, u32 spill_every) {
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
@@ -290,7 +290,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
   u32 n_events = 0, n_makework = 0, n_iter = 0, fresh = 0, backoff = 250;
   const u64 t_start = global_ns();
   u64 t_idle = 0, last_out = ~0ull;           // watchdog: no change of the outstanding count for deadline_ns while idle -> error
-  bool done = false; u32 inner_used = 0, n_top = 0;
+  bool done = false; u32 inner_used = 0;
   for (;;) {
     // Lockstep: the warps of a CTA pass the loop top together, so that they run the same event code at the same time
     // and an instruction line fetched for one warp serves the others from the SM's instruction cache (the loop is
@@ -307,9 +307,6 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       if (__syncthreads_and((done || (MODE == 0 && R.kmode && primary_done)) ? 1 : 0)) lockstep = 0;
       done = false;
     }
-    // stress option (tests): hand a runnable link to the global queues every spill_every-th pass, so that the spill /
-    // fetch machinery is exercised even when the stash never overflows
-    if (spill_every && s.nfull() > 0 && (++n_top % spill_every) == 0) spill_link(w, s.full(0), 0);
     int l = -1, fi = -1;
     if (s.nfull() > 0) { fi = s.nfull() - 1; l = s.full(fi); }
     else {
@@ -421,6 +418,11 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       if (dm) stash_insert(w, EV_SOURCE, slot, died);
       stash_insert(w, EV_STEP, slot, live);
       if ((++n_iter & 63u) == 0 && delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+      if (!lockstep && s.nfull() >= 2) {          // no lockstep (tail, or switched off): hand a full link to a starved warp
+        u64 st = 0;
+        if (w.lane == 0) st = ld_vol(R.starved);
+        if (__shfl_sync(FULL, st, 0) > 0) spill_link(w, s.full(0), 0);
+      }
       continue;
     }
     if (MODE == 2) {
