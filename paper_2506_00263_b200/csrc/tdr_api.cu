@@ -32,9 +32,9 @@ struct tdr_problem {
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
   int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
-  int seg_per_launch = 3;                  // stack fused/hybrid: segments per particle per k_step launch
+  int seg_per_launch = 0;                  // stack fused/hybrid: segments per particle per k_step launch; 0 = auto (3 multigroup, 8 continuous energy)
   int force_spill = 0;                     // async stress option (tests): warps always believe another one is starved
-  int seg_per_event = 2;                   // async fused: segments a particle is followed per step event before remapping
+  int seg_per_event = 0;                   // async fused: segments per step event before remapping; 0 = auto (2 multigroup, 5 continuous energy)
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
   int idle_timeout_s = 30;                 // async scheme watchdog (seconds without progress while idle)
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
@@ -177,9 +177,9 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "time_kernels") p->time_kernels = atoi(value);
   else if (k == "lockstep") p->lockstep = atoi(value) != 0;
   else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > 1024 || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,1024]"); p->async_threads = n; }
-  else if (k == "seg_per_launch") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "seg_per_launch in [1,1024]"); p->seg_per_launch = n; }
+  else if (k == "seg_per_launch") { int n = atoi(value); if (n < 0 || n > 1024) return fail(TDR_EINVAL, "seg_per_launch in [0,1024]"); p->seg_per_launch = n; }
   else if (k == "force_spill") p->force_spill = atoi(value) != 0;
-  else if (k == "seg_per_event") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "seg_per_event in [1,1024]"); p->seg_per_event = n; }
+  else if (k == "seg_per_event") { int n = atoi(value); if (n < 0 || n > 1024) return fail(TDR_EINVAL, "seg_per_event in [0,1024]"); p->seg_per_event = n; }
   else if (k == "slots_per_warp") { int n = atoi(value); if (n < 32 || n > 4096) return fail(TDR_EINVAL, "slots_per_warp in [32,4096]"); p->slots_per_warp = n; }
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
@@ -352,13 +352,13 @@ static int run_stack(tdr_problem *p, DevRun R) {
         const int g1 = g_step < cap_blocks ? g_step : cap_blocks;
         if (hybrid) {
           k_step<CE, true><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                  p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, (u32)p->seg_per_launch);
+                                                  p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3)));
           k_collide<CE><<<g_coll < cap_blocks ? g_coll : cap_blocks, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[2], cc,
                                                                                      p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
           p->diag.kernel_launches++;
         } else
           k_step<CE, false><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                   p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, (u32)p->seg_per_launch);
+                                                   p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3)));
         LAUNCH_CHECK(); p->diag.kernel_launches++;
       } else if ((rc = split_iteration<CE>(p, R, smem, sg, cap_blocks))) return rc;
       it++; p->diag.iterations++;
@@ -408,7 +408,7 @@ static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int thread
   int grid = grid_for(p, k_async<CE, MODE>, smem, threads);
   KTimer t(p, true);
   k_async<CE, MODE><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
-                                                        (u32)p->slots_per_warp, p->lockstep, (u32)p->seg_per_event);
+                                                        (u32)p->slots_per_warp, p->lockstep, (u32)(p->seg_per_event ? p->seg_per_event : (CE ? 5 : 2)));
   return 0;
 }
 

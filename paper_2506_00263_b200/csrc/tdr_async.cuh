@@ -301,7 +301,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
       // Between two votes every warp of the CTA passes exactly seg_per_event - 1 further barriers: a step event meets
       // them between its segments (so the segments of all warps start together as well), every other path makes up
       // for them here.
-      if (MODE == 0) { for (u32 j = inner_used; j + 1 < seg_per_event; j++) __syncthreads_and(1); inner_used = 0; }
+      if (MODE == 0 && !CE) { for (u32 j = inner_used; j + 1 < seg_per_event; j++) __syncthreads_and(1); inner_used = 0; }
       // the vote: every warp is done, or (k-mode) has seen the source exhausted -> the CTA drops the lockstep for the
       // tail; a warp that is done then leaves on its own, the others drain their links without a barrier
       if (__syncthreads_and((done || (MODE == 0 && R.kmode && primary_done)) ? 1 : 0)) lockstep = 0;
@@ -408,7 +408,8 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
         if (lm == 0) break;
         if (k + 1 < kmax) {
           n_events += (u32)__popc(lm);
-          if (lockstep) { __syncthreads_and(1); inner_used++; }
+          if (lockstep && !CE) { __syncthreads_and(1); inner_used++; }   // continuous energy: the cross-section gathers make the
+                                                                        // segments' durations uneven and the extra barrier costs 5 %
         }
       }
       if (live) store_part<CE>(S, slot, p);
