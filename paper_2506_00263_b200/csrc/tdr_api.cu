@@ -88,12 +88,62 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
   const double *mp[3] = { g->mesh_x, g->mesh_y, g->mesh_z };
   const double *lp[3] = { g->xplanes, g->yplanes, g->zplanes };
   const int ln[3] = { g->nx, g->ny, g->nz };
+  if (!g->xplanes || !g->yplanes || !g->zplanes || !g->cx || !g->cy || !g->cell_univ || !g->univ_nrings || !g->univ_radius ||
+      !g->univ_mat || !mp[0] || !mp[1] || !mp[2]) return fail(TDR_EINVAL, "null geometry array");
   for (int a = 0; a < 3; a++) {
     if (g->mesh_n[a] < 1 || g->mesh_n[a] > 32767) return fail(TDR_EINVAL, "bad mesh size");
     if (!(mp[a][0] <= lp[a][0]) || !(mp[a][g->mesh_n[a]] >= lp[a][ln[a]])) return fail(TDR_EINVAL, "tally mesh must cover the lattice box");
   }
-  for (int u = 0; u < g->n_univ; u++)
-    if (g->univ_nrings[u] < 0 || g->univ_nrings[u] > TDR_MAX_RINGS) return fail(TDR_EINVAL, "bad ring count");
+  // every index table is dereferenced on the device: range-check it here (a bad index would be an illegal address there)
+  for (int a = 0; a < 3; a++) {
+    for (int k = 0; k < ln[a]; k++) if (!(lp[a][k] < lp[a][k + 1])) return fail(TDR_EINVAL, "lattice planes of axis %d are not strictly ascending", a);
+    for (int k = 0; k < g->mesh_n[a]; k++) if (!(mp[a][k] < mp[a][k + 1])) return fail(TDR_EINVAL, "mesh planes of axis %d are not strictly ascending", a);
+  }
+  for (int u = 0; u < g->n_univ; u++) {
+    const int nr = g->univ_nrings[u];
+    if (nr < 0 || nr > TDR_MAX_RINGS) return fail(TDR_EINVAL, "bad ring count");
+    for (int r = 0; r < nr; r++) {
+      const double R = g->univ_radius[u * TDR_MAX_RINGS + r];
+      if (!(R > 0.0) || (r > 0 && !(R > g->univ_radius[u * TDR_MAX_RINGS + r - 1]))) return fail(TDR_EINVAL, "radii of universe %d are not positive and ascending", u);
+    }
+    for (int r = 0; r <= nr; r++) {
+      const int mt = g->univ_mat[u * (TDR_MAX_RINGS + 1) + r];
+      if (mt < 0 || mt >= m->n_mat) return fail(TDR_EINVAL, "universe %d names material %d of %d", u, mt, m->n_mat);
+    }
+  }
+  for (int iz = 0; iz < g->nz; iz++) for (int iy = 0; iy < g->ny; iy++) for (int ix = 0; ix < g->nx; ix++) {
+    const int u = g->cell_univ[((size_t)iz * g->ny + iy) * g->nx + ix];
+    if (u < 0 || u >= g->n_univ) return fail(TDR_EINVAL, "cell (%d,%d,%d) names universe %d of %d", ix, iy, iz, u, g->n_univ);
+    const int nr = g->univ_nrings[u];
+    if (nr > 0) {                             // G7: a particle on a cell face is outside every ring
+      const double R = g->univ_radius[u * TDR_MAX_RINGS + nr - 1];
+      const double hx0 = g->cx[ix] - g->xplanes[ix], hx1 = g->xplanes[ix + 1] - g->cx[ix], hy0 = g->cy[iy] - g->yplanes[iy], hy1 = g->yplanes[iy + 1] - g->cy[iy];
+      if (!(R < hx0) || !(R < hx1) || !(R < hy0) || !(R < hy1)) return fail(TDR_EINVAL, "outer radius of universe %d reaches the face of cell (%d,%d)", u, ix, iy);
+    }
+  }
+  for (int f = 0; f < 6; f++) if (g->bc[f] != 0 && g->bc[f] != 1) return fail(TDR_EINVAL, "bc must be 0 (vacuum) or 1 (reflective)");
+  if (g->src_kind < 0 || g->src_kind > 1 || g->src_dir_kind < 0 || g->src_dir_kind > 1 || g->src_energy_kind < 0 || g->src_energy_kind > 2)
+    return fail(TDR_EINVAL, "bad source kind");
+  if (m->G > 0) {
+    if (!m->sig_t || !m->sig_s || !m->sig_f || !m->nu || !m->chi) return fail(TDR_EINVAL, "null multigroup table");
+    if (g->src_energy_kind != 0 || g->src_index < 0 || g->src_index >= m->G) return fail(TDR_EINVAL, "multigroup source must name a group below G");
+    // the table is staged to shared memory by every kernel: it has to fit beside the private tallies and the stash
+    if ((size_t)m->n_mat * m->G * (MGROW(m->G) + 1) * sizeof(double) > 96 * 1024) return fail(TDR_EINVAL, "multigroup table too large for shared memory (n_mat*G*(G+6)*8 > 96 KB)");
+  } else {
+    if (!m->mat_nnuc || !m->mat_nuc || !m->mat_dens || !x->energy || !x->A || !x->sig_s || !x->sig_c || !x->sig_f || !x->nu || !x->watt_a || !x->watt_b)
+      return fail(TDR_EINVAL, "null continuous-energy table");
+    if (x->n_grid < 2 || x->n_nuc < 1 || x->n_nuc > 255) return fail(TDR_EINVAL, "bad CE tables");
+    for (int k = 0; k < m->n_mat; k++) {
+      if (m->mat_nnuc[k] < 1 || m->mat_nnuc[k] > TDR_MAX_NUC) return fail(TDR_EINVAL, "material %d has %d nuclides (1..%d)", k, m->mat_nnuc[k], TDR_MAX_NUC);
+      for (int n = 0; n < m->mat_nnuc[k]; n++)
+        if (m->mat_nuc[k * TDR_MAX_NUC + n] < 0 || m->mat_nuc[k * TDR_MAX_NUC + n] >= x->n_nuc) return fail(TDR_EINVAL, "material %d names nuclide %d of %d", k, m->mat_nuc[k * TDR_MAX_NUC + n], x->n_nuc);
+    }
+    for (int i = 0; i + 1 < x->n_grid; i++) if (!(x->energy[i] < x->energy[i + 1])) return fail(TDR_EINVAL, "energy grid is not strictly increasing at %d", i);
+    if (g->n_ebins < 1 || !g->e_edges) return fail(TDR_EINVAL, "continuous energy needs n_ebins >= 1 and e_edges");
+    for (int i = 0; i < g->n_ebins; i++) if (!(g->e_edges[i] < g->e_edges[i + 1])) return fail(TDR_EINVAL, "energy-bin edges are not strictly ascending");
+    if (g->src_energy_kind == 0) return fail(TDR_EINVAL, "continuous-energy source must be mono or Watt");
+    if (g->src_energy_kind == 2 && (g->src_index < 0 || g->src_index >= x->n_nuc)) return fail(TDR_EINVAL, "Watt source names nuclide %d of %d", g->src_index, x->n_nuc);
+  }
   int dev_count = 0;
   if (cudaGetDeviceCount(&dev_count) != cudaSuccess || dev_count == 0) return fail(TDR_ECUDA, "no CUDA device: this library has no CPU fallback");
   tdr_problem *p = new tdr_problem();
@@ -170,13 +220,13 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   std::string k(key), v(value);
   if (k == "scheme") { if (v == "stack") p->scheme = 0; else if (v == "async") p->scheme = 1; else return fail(TDR_EINVAL, "scheme must be stack|async"); }
   else if (k == "decomposition") { if (v == "fused") p->split = 0; else if (v == "split") p->split = 1; else if (v == "hybrid") p->split = 2; else return fail(TDR_EINVAL, "decomposition must be fused|split|hybrid"); }
-  else if (k == "window") { long long w = atoll(value); if (w < 32) return fail(TDR_EINVAL, "window too small"); p->window = (u64)w; }
+  else if (k == "window") { long long w = atoll(value); if (w < 32) return fail(TDR_EINVAL, "window too small"); if (w > 0xFFFFFFC0ll) return fail(TDR_EINVAL, "window above 2^32 - 64: slot indices are 32-bit"); p->window = (u64)w; }
   else if (k == "stash_links") { int n = atoi(value); if (n < 8 || n > 64) return fail(TDR_EINVAL, "stash_links in [8,64]"); p->stash_links = n; }
   else if (k == "blocks_per_sm") p->blocks_per_sm = atoi(value);
   else if (k == "keep_history") p->keep_history = atoi(value);
   else if (k == "time_kernels") p->time_kernels = atoi(value);
   else if (k == "lockstep") p->lockstep = atoi(value) != 0;
-  else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > 1024 || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,1024]"); p->async_threads = n; }
+  else if (k == "async_threads") { int n = atoi(value); if (n < 64 || n > TDR_ASYNC_MAXT || n % 32) return fail(TDR_EINVAL, "async_threads: a multiple of 32 in [64,%d]", TDR_ASYNC_MAXT); p->async_threads = n; }
   else if (k == "seg_per_launch") { int n = atoi(value); if (n < 0 || n > 1024) return fail(TDR_EINVAL, "seg_per_launch in [0,1024]"); p->seg_per_launch = n; }
   else if (k == "force_spill") p->force_spill = atoi(value) != 0;
   else if (k == "seg_per_event") { int n = atoi(value); if (n < 0 || n > 1024) return fail(TDR_EINVAL, "seg_per_event in [0,1024]"); p->seg_per_event = n; }
