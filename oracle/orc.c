@@ -476,12 +476,12 @@ static void transport(ctx *c, part *q) {
     }
     size_t bin = 0;
     if (e >= 0) bin = ((((size_t)q->mz * p->mesh_n[1] + q->my) * p->mesh_n[0]) + q->mx) * p->n_e + e;
-    if (c->active && e >= 0) c->flux[bin] += fixp(p, d);
+    if (c->active && e >= 0 && __builtin_add_overflow(c->flux[bin], fixp(p, d), &c->flux[bin])) { c->err = ORC_EOVERFLOW; return; }   /* N5 */
     if (c->kmode) c->P += fixp(p, d * nsf);
     if (collide) {
       /* T6 */
       q->ncoll += 1; c->tot[ORC_T_NCOLL] += 1;
-      if (c->active && e >= 0) c->coll[bin] += fixp(p, 1.0);
+      if (c->active && e >= 0 && __builtin_add_overflow(c->coll[bin], fixp(p, 1.0), &c->coll[bin])) { c->err = ORC_EOVERFLOW; return; }
       if (c->kmode) c->Pc += fixp(p, nsf / St);
       int kind;                                                         /* 0 scatter 1 capture 2 fission */
       int fnuc = 0; double nu = 0.0; int src = mat;
@@ -591,7 +591,8 @@ static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, in
     {
       if (c.err && !out->err) out->err = c.err;
       if (!c.err) {
-        for (uint64_t b = 0; b < p->n_bins; b++) { p->flux[b] += c.flux[b]; p->coll[b] += c.coll[b]; }
+        for (uint64_t b = 0; b < p->n_bins; b++)                 /* N5: every tally sum is checked against int64 */
+          if (__builtin_add_overflow(p->flux[b], c.flux[b], &p->flux[b]) || __builtin_add_overflow(p->coll[b], c.coll[b], &p->coll[b])) out->err = ORC_EOVERFLOW;
         for (int f = 0; f < 6; f++) p->leak[f] += c.leak[f];
         for (int t = 0; t < ORC_T_COUNT; t++) p->totals[t] += c.tot[t];
         out->P += c.P; out->Pc += c.Pc;

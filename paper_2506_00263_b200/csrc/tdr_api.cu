@@ -40,6 +40,8 @@ struct tdr_problem {
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
   int drain_below = 65536;                 // stack scheme, k-mode: population below which the tail is drained in one launch
   int sync_every = 6;                      // stack scheme: remap iterations launched per counter read-back
+  u64 bank_cap_opt = 0;                    // tests: fission-bank capacity in sites (0 = 2.5 n + 4096)
+  u64 arena_links_opt = 0;                 // tests: global link arena of the asynchronous scheme (0 = 2 W/32 + 4096)
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
   // carved pointers (valid during/after a run)
@@ -234,6 +236,8 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
   else if (k == "drain_below") { int n = atoi(value); if (n < 0) return fail(TDR_EINVAL, "drain_below >= 0"); p->drain_below = n; }
+  else if (k == "bank_cap") p->bank_cap_opt = strtoull(value, nullptr, 10);
+  else if (k == "arena_links") p->arena_links_opt = strtoull(value, nullptr, 10);
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -268,11 +272,11 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   DevOut o;
   o.flux = c.take<u64>(p->dp.n_bins); o.coll = c.take<u64>(p->dp.n_bins); o.leak = c.take<u64>(6);
   o.totals = c.take<u64>(TDR_T_COUNT); o.PPc = c.take<u64>(2); o.err = c.take<int>(1);
-  u64 bank_cap = 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + (1ull << 20);
+  u64 bank_cap = p->bank_cap_opt ? p->bank_cap_opt : 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + (1ull << 20);
   tdr_site *bank = c.take<tdr_site>(bank_cap), *src = c.take<tdr_site>(src_cap), *sec = c.take<tdr_site>(sec_cap);
   u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
   u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
-  AsyncMem am; async_layout(c, W, sec_cap, am);
+  AsyncMem am; async_layout(c, W, sec_cap, p->arena_links_opt, am);
   if (assign) {
     p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
     p->bank = bank; p->srcbank = src; p->sec = sec; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;

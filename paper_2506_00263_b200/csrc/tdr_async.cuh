@@ -29,8 +29,8 @@ enum { AC_GWORK = 0, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_EVENTS, AC_DBG = 8, 
 struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *actr; u64 *sec_flag; };
 
 template <class C>
-static void async_layout(C &c, u64 W, u64 sec_cap, AsyncMem &am) {
-  am.n_links = 2 * (W / 32) + 4096;
+static void async_layout(C &c, u64 W, u64 sec_cap, u64 n_links_opt, AsyncMem &am) {
+  am.n_links = n_links_opt ? n_links_opt : 2 * (W / 32) + 4096;
   am.links = c.template take<GLink>(am.n_links);
   am.q_empty = c.template take<u64>(AQ); am.q_work = c.template take<u64>(AQ);
   am.actr = c.template take<u64>(AC_COUNT);

@@ -128,6 +128,91 @@ def slab(sig_t, L, n=100000, seed=1):
     return Problem("slab", geo, mats, None, "fixed", n, seed=seed)
 
 
+def slab_mesh(sig_t, sig_s, L, axis=0, direction=(1.0, 0.0, 0.0), start=0.0, lattice=None, mesh=None, n=100000, seed=1):
+    """1-group slab 0 < r[axis] < L (vacuum faces, infinite in the other two axes), mono-directional point source at
+    r[axis] = start; `lattice` = interior lattice planes along the axis, `mesh` = tally planes along the axis (they need
+    not coincide with the lattice planes)."""
+    planes = [[-INF, INF], [-INF, INF], [-INF, INF]]
+    planes[axis] = [0.0] + list(lattice or []) + [L]
+    ncell = len(planes[axis]) - 1
+    mp = [[-INF, INF], [-INF, INF], [-INF, INF]]
+    mp[axis] = list(mesh) if mesh is not None else [0.0, L]
+    src = [0.0, 0.0, 0.0]
+    src[axis] = start
+    geo = geometry(planes[0], planes[1], planes[2], [0] * ncell, [((), (0,))], [0] * 6, mesh=tuple(mp),
+                   src_lo=tuple(src), src_dir=direction)
+    mats = mg_materials([[sig_t]], [[[sig_s]]], [[0.0]], [[0.0]], [[1.0]])
+    return Problem("slab_mesh", geo, mats, None, "fixed", n, seed=seed)
+
+
+def two_region(kind="pin", n=200000, seed=1):
+    """Volume-ratio pin: one group, the same S_t = 1.0 and S_s = 0.7 everywhere, uniform isotropic box
+    source, all faces reflective, so the flux is flat; absorption in the fuel rings is booked as fission with nu = 0
+    (no children), in the moderator as capture, so n_fis / (n_fis + n_abs) = fuel volume fraction.
+    kind: "pin" (cfg1's cell), "lattice" (3 x 3 cells: lattice-plane crossings reset the ring), "zones" (two axial zones
+    with different universes: a z crossing re-locates the ring), "rings" (two nested rings, fuel in the annulus)."""
+    h, R = 0.63, 0.54
+    mats = mg_materials([[1.0], [1.0]], [[[0.7]], [[0.7]]], [[0.3], [0.0]], [[0.0], [0.0]], [[1.0], [1.0]])
+    pi = float(np.pi)
+    if kind == "pin":
+        geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((R,), (0, 1))], [1, 1, 1, 1, 0, 0],
+                       src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0))
+        frac = pi * R * R / (4 * h * h)
+    elif kind == "lattice":
+        xp = [-3 * h, -h, h, 3 * h]
+        geo = geometry(xp, xp, [-INF, INF], [0] * 9, [((R,), (0, 1))], [1, 1, 1, 1, 0, 0],
+                       src_kind=1, src_lo=(-3 * h, -3 * h, 0.0), src_hi=(3 * h, 3 * h, 0.0))
+        frac = pi * R * R / (4 * h * h)
+    elif kind == "zones":
+        R2 = 0.30
+        geo = geometry([-h, h], [-h, h], [0.0, 1.0, 2.5], [0, 1], [((R,), (0, 1)), ((R2,), (0, 1))], [1] * 6,
+                       src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 2.5))
+        frac = (pi * R * R * 1.0 + pi * R2 * R2 * 1.5) / (4 * h * h * 2.5)
+    elif kind == "rings":
+        R1 = 0.25
+        geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((R1, R), (1, 0, 1))], [1, 1, 1, 1, 0, 0],
+                       src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0))
+        frac = pi * (R * R - R1 * R1) / (4 * h * h)
+    else:
+        raise ValueError(kind)
+    p = Problem("two_region_" + kind, geo, mats, None, "fixed", n, seed=seed)
+    p.notes["fuel_volume_fraction"] = frac
+    return p
+
+
+def ce_two_nuclide_medium(order=(0, 1), mode="k", n=20000, n_inactive=3, n_active=17, seed=1, scatter=True, n_ebins=None):
+    """Infinite medium of two nuclides with energy-independent cross sections (CE collision pin): nuclide 0 = scatterer /
+    absorber (A = 12), nuclide 1 = fissile (A = 200, nu = 2, Watt a = 0.9e6, b = 2.0e-6).  `order` = the order in which
+    the material lists them (results must not depend on it statistically)."""
+    n_grid = 64
+    E = np.exp(np.linspace(np.log(1e-5), np.log(2e7), n_grid))
+    E[0], E[-1] = 1e-5, 2e7
+    s = np.array([[2.0], [1.0]]) * (1.0 if scatter else 0.0) * np.ones((2, n_grid))
+    c = np.array([[1.0], [0.5]]) * np.ones((2, n_grid))
+    f = np.array([[0.0], [1.5]]) * np.ones((2, n_grid))
+    xs = dict(n_grid=n_grid, n_nuc=2, energy=_f64(E), A=_f64([12.0, 200.0]), sig_s=_f64(s), sig_c=_f64(c), sig_f=_f64(f),
+              nu=_f64([0.0, 2.0]), watt_a=_f64([1.0, 0.9e6]), watt_b=_f64([1.0, 2.0e-6]))
+    dens = {0: 0.5, 1: 0.3}
+    edges = [1e-5, 2e7] if n_ebins is None else n_ebins
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, e_edges=edges,
+                   src_energy=("watt", 1) if mode == "k" else ("mono", 1e6))
+    mats = ce_materials([[(order[0], dens[order[0]]), (order[1], dens[order[1]])]])
+    p = Problem("ce_two_nuclide", geo, mats, xs, mode, n, n_inactive, n_active, seed)
+    p.notes.update(N=dens, sig_s=(2.0 if scatter else 0.0, 1.0 if scatter else 0.0), sig_c=(1.0, 0.5), sig_f=(0.0, 1.5), nu=2.0,
+                   watt=(0.9e6, 2.0e-6))
+    return p
+
+
+def ce_lerp_absorber(E0, n=100000, seed=1):
+    """Pure absorber whose capture cross section is tabulated on a COARSE grid, mono-energetic source between grid points
+    (or outside the grid): pins the X2 interpolation and clamping.  sigma_c = 8, 2, 4, 1 b at 1, 10, 100, 1000 eV; N = 0.4."""
+    xs = dict(n_grid=4, n_nuc=1, energy=_f64([1.0, 10.0, 100.0, 1000.0]), A=_f64([10.0]), sig_s=_f64(np.zeros((1, 4))),
+              sig_c=_f64([[8.0, 2.0, 4.0, 1.0]]), sig_f=_f64(np.zeros((1, 4))), nu=_f64([0.0]), watt_a=_f64([1.0]), watt_b=_f64([1.0]))
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, e_edges=[1e-3, 1e5],
+                   src_energy=("mono", E0))
+    return Problem("ce_lerp_absorber", geo, ce_materials([[(0, 0.4)]]), xs, "fixed", n, seed=seed)
+
+
 def _mg_material(rng, G, kind):
     """One synthetic G-group material (recipe: DESIGN.md section 4, cfg1)."""
     sig_t = rng.uniform(0.2, 2.0, G)

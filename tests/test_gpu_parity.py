@@ -131,3 +131,79 @@ def test_async_spill_and_fetch_through_the_global_queues(decomp):
         assert d["fetches"] == d["spills"], d
         total += d["spills"]
     assert total > 0
+
+
+# ------------------------------------------------------------------ round 2: holes named by the round-1 review
+@pytest.mark.parametrize("decomp", ["fused", "hybrid"])
+def test_stack_remap_loop_runs_to_extinction_without_the_tail_drain(decomp):
+    """drain_below = 0: the k-mode stack scheme never hands the tail to k_drain, so the remap loop itself (rotating
+    counters, the collide-stack hand-off of the hybrid, many iterations of a dwindling population) runs to the last particle."""
+    for p in (W.cfg1(n=30011, n_inactive=1, n_active=2), W.cfg4(n=20011, n_inactive=1, n_active=1)):
+        o, g, d = run_both(p, scheme="stack", decomposition=decomp, drain_below=0)
+        assert_same(o, g, f"{p.name}/stack/{decomp}/drain_below=0")
+        assert d["iterations"] > 50, d
+
+
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+def test_cfg2_and_cfg4_at_a_million_per_generation(scheme, decomp):
+    """The two large workloads at 1e6 particles per generation (beyond the 2^20-slot window, so make_work refills run),
+    every scheme and decomposition: totals with the history digest, all tallies, per-generation sums, the bank."""
+    for p in (W.cfg2(n=1000003, n_inactive=1, n_active=1), W.cfg4(n=1000003, n_inactive=1, n_active=1)):
+        o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+        assert_same(o, g, f"{p.name}@1e6/{scheme}/{decomp}")
+
+
+@pytest.mark.parametrize("scheme", ["stack", "async"])
+def test_full_size_split_decomposition(scheme):
+    """The five-event decomposition at BASELINE's full per-generation size of cfg1 (1e6; 4 generations)."""
+    p = W.cfg1(n_inactive=1, n_active=3)
+    o, g, d = run_both(p, scheme=scheme, decomposition="split")
+    assert_same(o, g, f"full-size cfg1/{scheme}/split")
+
+
+def test_capacity_and_lost_particle_errors_are_reported():
+    from paper_2506_00263_b200 import tdr
+    # fission bank far too small -> TDR_ECAPACITY (-4), under both schemes
+    for scheme in ("stack", "async"):
+        P = tdr.Problem(W.cfg1(n=20000, n_inactive=1, n_active=1), scheme=scheme, bank_cap=100)
+        with pytest.raises(tdr.TdrError) as e:
+            P.run()
+        assert e.value.code == -4, e.value
+        P.close()
+    # asynchronous scheme: forced spills with a global link arena of 8 links -> TDR_ECAPACITY
+    P = tdr.Problem(W.cfg1(n=300007, n_inactive=1, n_active=1), scheme="async", decomposition="hybrid", force_spill=1, lockstep=0,
+                    slots_per_warp=256, arena_links=8)
+    with pytest.raises(tdr.TdrError) as e:
+        P.run()
+    assert e.value.code == -4, e.value
+    P.close()
+    # a void with no boundary in reach: no finite distance -> TDR_ELOST (-5), as the oracle says too
+    void = W.infinite_medium([0.0], [[0.0]], n=1000)
+    for scheme in ("stack", "async"):
+        P = tdr.Problem(void, scheme=scheme)
+        with pytest.raises(tdr.TdrError) as e:
+            P.run()
+        assert e.value.code == -5, e.value
+        P.close()
+    from oracle import orc
+    with pytest.raises(RuntimeError, match="-5"):
+        orc.run(void)
+    # the library is usable after an error
+    o, g, _ = run_both(W.cfg0(n=1000))
+    assert_same(o, g, "after errors")
+
+
+def test_results_do_not_depend_on_the_launch_configuration():
+    """Order independence (SURVEY section 4 tier 5): the same problem under different grid sizes, CTA sizes, windows and
+    stash sizes gives the same integers."""
+    from oracle import orc
+    p = W.cfg1(n=100003, n_inactive=1, n_active=2)
+    o = orc.run(p)
+    from paper_2506_00263_b200 import tdr
+    for kw in (dict(scheme="stack", blocks_per_sm=1), dict(scheme="stack", blocks_per_sm=2), dict(scheme="stack", blocks_per_sm=4, window=50000),
+               dict(scheme="async", async_threads=256), dict(scheme="async", async_threads=512, stash_links=16),
+               dict(scheme="async", async_threads=128, lockstep=0, slots_per_warp=64), dict(scheme="async", decomposition="split", async_threads=256)):
+        P = tdr.Problem(p, **kw)
+        g = P.run()
+        P.close()
+        assert_same(o, g, str(kw))

@@ -119,9 +119,9 @@ def test_ce_scatter_kinematics(A):
     assert abs(xi.mean() - xi_ref) < 4 * xi.std() / math.sqrt(n)
     assert abs(mu.mean() - 2 / (3 * A)) < 4 * mu.std() / math.sqrt(n)
     assert Eo.value <= 2.0e6 * (1 + 1e-15)
-    # azimuth uniform: component of the outgoing direction perpendicular to din averages to 0
-    perp = np.cross(din[100:], [0, 0, 1.0])
-    assert xi.max() <= -math.log(alpha) + 1e-9 if A > 1 else True
+    # (the azimuth about the incoming direction is pinned in test_oracle_pins_transport.py)
+    if A > 1:
+        assert xi.max() <= -math.log(alpha) + 1e-9
 
 
 # ------------------------------------------------------------------ geometry / lookup (G4, X2)
