@@ -132,6 +132,19 @@ int tdr_bind_workspace(tdr_problem *, void *device_ptr, uint64_t bytes, void *cu
 int tdr_run_fixed_source(tdr_problem *, uint64_t n_particles, uint64_t seed);
 /* D2: power iteration with population control; tallies over active generations. */
 int tdr_run_k_eigenvalue(tdr_problem *, uint64_t n_particles, uint32_t n_inactive, uint32_t n_active, uint64_t seed);
+/* D2 in steps, for ONE k-eigenvalue problem shared by several GPUs (one process each; the paper's counterpart is
+ * MPI replication over 4 V100s).  Every process holds a contiguous share of the source:
+ *   tdr_k_begin(first_id, n_local, n_gen, seed)             generation-0 ids first_id .. first_id + n_local - 1
+ *   tdr_k_generation(gen, active, k_prev, last, sums)       runs the local share; sums = { P, Pc, N_local, M_local } (fixed point)
+ *   -- the caller adds the four sums over all processes (one 32-byte all-reduce) and forms k_g = P 2^-S / N, pr = N_target / M --
+ *   tdr_k_population_control(gen_next, pr, &n_next)         controls the LOCAL bank with the GLOBAL ratio pr; sites stay where they are
+ *   tdr_k_end(...)                                          stores the global per-generation results for tdr_read_tallies
+ * Results are bit-identical for any number of shares; tdr_run_k_eigenvalue is this loop with one share.  HOST pointers. */
+int tdr_k_begin(tdr_problem *, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed);
+int tdr_k_generation(tdr_problem *, uint32_t gen, int active, double k_prev, int last, int64_t sums[4]);
+int tdr_k_population_control(tdr_problem *, uint32_t gen_next, double pr, uint64_t *n_next);
+int tdr_k_end(tdr_problem *, uint32_t n_gen, uint32_t n_inactive, const uint64_t *gen_n, const uint64_t *gen_m, const int64_t *gen_p,
+              const int64_t *gen_pc, const double *gen_k);
 int tdr_tally_sizes(const tdr_problem *, tdr_sizes *out);
 /* Copies device tallies into the caller's HOST buffers.  TDR_ESTATE before any run. */
 int tdr_read_tallies(const tdr_problem *, tdr_tallies *out);

@@ -173,6 +173,8 @@ int32_t orc_grid_index(const double *grid, int32_t n, double E) {
 }
 
 /* ------------------------------------------------------------------ problem */
+typedef struct { uint64_t *id; uint32_t *nseg, *ncoll; size_t n, cap; } histvec;   /* per-history records */
+
 struct orc_problem {
   int nx, ny, nz, bc[6], n_univ, mesh_n[3], by_group, n_e, S;
   double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges;
@@ -192,6 +194,8 @@ struct orc_problem {
   uint64_t n_hist, *hist_id; uint32_t *hist_nseg, *hist_ncoll;
   uint64_t n_bank; orc_site *bank;
   int ran;
+  /* D2 in steps: this process's source share, its bank, its history records */
+  uint64_t k_first, n_ksrc, n_kbank, kseed; orc_site *ksrc, *kbank; histvec khist;
 };
 
 static void *dup_mem(const void *src, size_t bytes) {
@@ -220,6 +224,7 @@ void orc_free_problem(orc_problem *p) {
   free(p->chicdf); free(p->nusigf); free(p->mat_nnuc); free(p->mat_nuc); free(p->mat_dens);
   free(p->grid); free(p->A); free(p->xs_s); free(p->xs_c); free(p->xs_f); free(p->nuc_nu);
   free(p->wa); free(p->wb);
+  free(p->ksrc); free(p->kbank); free(p->khist.id); free(p->khist.nseg); free(p->khist.ncoll);
   free(p);
 }
 
@@ -295,7 +300,6 @@ typedef struct {
 } part;
 
 typedef struct { orc_site *v; size_t n, cap; } sitevec;
-typedef struct { uint64_t *id; uint32_t *nseg, *ncoll; size_t n, cap; } histvec;
 
 typedef struct {
   const orc_problem *p;
@@ -361,7 +365,7 @@ static void birth_common(ctx *c, part *q, int src, int from_site) {
   c->tot[ORC_T_NBORN] += 1;
 }
 
-static void birth_primary(ctx *c, part *q, uint64_t i) {
+static void birth_primary(ctx *c, part *q, uint64_t i) {                /* i = source id (D1: first_id + index) */
   const orc_problem *p = c->p;
   q->id = i; q->depth = 0;
   double pos[3];
@@ -565,7 +569,7 @@ int orc_set_threads(int n) { g_threads = n > 0 ? n : 0; return g_threads ? g_thr
 typedef struct { __int128 P, Pc; sitevec bank; int err; } batch_out;
 
 /* one batch of histories: sources are primary indices [0,n_src) (sites == NULL) or sites[0..n_src) */
-static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, int active, double k_prev,
+static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, int active, double k_prev, uint64_t first_id,
                       uint64_t n_src, const orc_site *sites, int keep_hist, histvec *hist_all, batch_out *out) {
   int nt = g_threads ? g_threads : omp_get_max_threads();
   out->P = 0; out->Pc = 0; out->bank.v = NULL; out->bank.n = out->bank.cap = 0; out->err = 0;
@@ -579,7 +583,7 @@ static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, in
     for (uint64_t i = 0; i < n_src; i++) {
       if (c.err) continue;
       part q;
-      if (sites) birth_site(&c, &q, &sites[i]); else birth_primary(&c, &q, i);
+      if (sites) birth_site(&c, &q, &sites[i]); else birth_primary(&c, &q, first_id + i);
       transport(&c, &q);
       while (!c.err && c.stack.n > 0) {                 /* D1: secondaries, LIFO, to extinction */
         orc_site s = c.stack.v[--c.stack.n];
@@ -629,12 +633,13 @@ static int alloc_results(orc_problem *p, uint64_t n_gen) {
 
 static int fits_i64(__int128 v) { return v < ((__int128)1 << 63) && v > -((__int128)1 << 63); }
 
-int orc_run_fixed_source(orc_problem *p, uint64_t n, uint64_t seed) {
+/* D1 over the id range [first_id, first_id + n): one share of a source split over several processes */
+int orc_run_fixed_source_range(orc_problem *p, uint64_t first_id, uint64_t n, uint64_t seed) {
   if (!p) return ORC_EINVAL;
   int rc = alloc_results(p, 0); if (rc) return rc;
   histvec h; memset(&h, 0, sizeof h);
   batch_out o;
-  run_batch(p, seed, 0, 0, 1, 1.0, n, NULL, n <= 2000000, &h, &o);
+  run_batch(p, seed, 0, 0, 1, 1.0, first_id, n, NULL, n <= 2000000, &h, &o);
   free(o.bank.v);
   p->hist_id = h.id; p->hist_nseg = h.nseg; p->hist_ncoll = h.ncoll; p->n_hist = h.n;
   if (o.err) return o.err;
@@ -642,42 +647,62 @@ int orc_run_fixed_source(orc_problem *p, uint64_t n, uint64_t seed) {
   return ORC_OK;
 }
 
-int orc_run_k_eigenvalue(orc_problem *p, uint64_t n, uint32_t n_inactive, uint32_t n_active, uint64_t seed) {
-  if (!p || n == 0 || (uint64_t)n_inactive + n_active == 0 || (uint64_t)n_inactive + n_active > 65535) return ORC_EINVAL;
-  uint32_t n_gen = n_inactive + n_active;
+int orc_run_fixed_source(orc_problem *p, uint64_t n, uint64_t seed) { return orc_run_fixed_source_range(p, 0, n, seed); }
+
+/* D2 in steps, so that one problem can be shared by several processes: every process holds a contiguous
+ * share of the source, runs its generation, the (P, Pc, N, M) sums are added over the processes, and every process
+ * controls its own bank with the global p = N / M.  orc_run_k_eigenvalue is the same loop with one share. */
+int orc_k_begin(orc_problem *p, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed) {
+  if (!p || n_gen == 0 || n_gen > 65535) return ORC_EINVAL;
   int rc = alloc_results(p, n_gen); if (rc) return rc;
-  orc_site *src = NULL; uint64_t n_src = n;
-  double k_prev = 1.0;
-  histvec h; memset(&h, 0, sizeof h);
-  for (uint32_t g = 0; g < n_gen; g++) {
-    batch_out o;
-    int last = (g + 1 == n_gen);
-    run_batch(p, seed, g, 1, g >= n_inactive, k_prev, n_src, src, last && n_src <= 2000000, &h, &o);
-    if (o.err) { free(o.bank.v); free(src); return o.err; }
-    if (!fits_i64(o.P) || !fits_i64(o.Pc)) { free(o.bank.v); free(src); return ORC_EOVERFLOW; }
-    double k = ((double)(int64_t)o.P * (1.0 / p->scale)) / (double)n_src;       /* D2 */
-    p->gen_n[g] = n_src; p->gen_m[g] = o.bank.n; p->gen_p[g] = (int64_t)o.P; p->gen_pc[g] = (int64_t)o.Pc; p->gen_k[g] = k;
-    p->n_gen = g + 1;
-    if (o.bank.n == 0) { free(o.bank.v); free(src); return ORC_ESTATE; }
-    if (last) { p->bank = o.bank.v; p->n_bank = o.bank.n; break; }
-    /* population control: m = floor(N/M + xi) copies per site, unit weights */
-    double pr = (double)n / (double)o.bank.n;
-    sitevec nx; memset(&nx, 0, sizeof nx);
-    for (size_t s = 0; s < o.bank.n; s++) {
-      const orc_site *b = &o.bank.v[s];
-      int m = (int)floor(pr + orc_draw(seed, b->id, g + 1, 0, PUR_POPCTRL, 0));
-      if (m > 2048) m = 2048;
-      for (int r = 0; r < m; r++) {
-        orc_site cp = *b; cp.id = orc_derive_id(seed, b->id, g + 1, 0, 2048u + (uint32_t)r);
-        if (push_site(&nx, &cp)) { free(o.bank.v); free(src); free(nx.v); return ORC_ENOMEM; }
-      }
+  free(p->ksrc); free(p->kbank); p->ksrc = NULL; p->kbank = NULL; p->n_kbank = 0;
+  p->k_first = first_id; p->n_ksrc = n_local; p->kseed = seed;
+  memset(&p->khist, 0, sizeof p->khist);
+  return ORC_OK;
+}
+
+/* one generation over this process's share; sums = { P, Pc, N_local, M_local } */
+int orc_k_generation(orc_problem *p, uint32_t gen, int active, double k_prev, int keep_hist, int64_t sums[4]) {
+  if (!p || !sums) return ORC_EINVAL;
+  batch_out o;
+  free(p->kbank); p->kbank = NULL; p->n_kbank = 0;
+  run_batch(p, p->kseed, gen, 1, active, k_prev, p->k_first, p->n_ksrc, p->ksrc, keep_hist && p->n_ksrc <= 2000000, &p->khist, &o);
+  if (o.err) { free(o.bank.v); return o.err; }
+  if (!fits_i64(o.P) || !fits_i64(o.Pc)) { free(o.bank.v); return ORC_EOVERFLOW; }
+  p->kbank = o.bank.v; p->n_kbank = o.bank.n;
+  sums[0] = (int64_t)o.P; sums[1] = (int64_t)o.Pc; sums[2] = (int64_t)p->n_ksrc; sums[3] = (int64_t)o.bank.n;
+  return ORC_OK;
+}
+
+/* population control of this process's bank with the global ratio pr = N / M: m = floor(pr + xi) copies per site */
+int orc_k_popctrl(orc_problem *p, uint32_t gen_next, double pr, uint64_t *n_next) {
+  if (!p || !n_next) return ORC_EINVAL;
+  sitevec nx; memset(&nx, 0, sizeof nx);
+  for (size_t s = 0; s < p->n_kbank; s++) {
+    const orc_site *b = &p->kbank[s];
+    int m = (int)floor(pr + orc_draw(p->kseed, b->id, gen_next, 0, PUR_POPCTRL, 0));
+    if (m > 2048) m = 2048;
+    for (int r = 0; r < m; r++) {
+      orc_site cp = *b; cp.id = orc_derive_id(p->kseed, b->id, gen_next, 0, 2048u + (uint32_t)r);
+      if (push_site(&nx, &cp)) { free(nx.v); return ORC_ENOMEM; }
     }
-    free(o.bank.v); free(src);
-    src = nx.v; n_src = nx.n; k_prev = k;
-    if (n_src == 0) return ORC_ESTATE;
   }
-  free(src);
-  p->hist_id = h.id; p->hist_nseg = h.nseg; p->hist_ncoll = h.ncoll; p->n_hist = h.n;
+  free(p->ksrc); p->ksrc = nx.v; p->n_ksrc = nx.n;
+  *n_next = nx.n;
+  return ORC_OK;
+}
+
+/* store the per-generation results (global sums) and close the run; the last bank stays readable */
+int orc_k_end(orc_problem *p, uint32_t n_gen, uint32_t n_inactive, const uint64_t *gen_n, const uint64_t *gen_m, const int64_t *gen_p,
+              const int64_t *gen_pc, const double *gen_k) {
+  if (!p) return ORC_EINVAL;
+  for (uint32_t g = 0; g < n_gen; g++) { p->gen_n[g] = gen_n[g]; p->gen_m[g] = gen_m[g]; p->gen_p[g] = gen_p[g]; p->gen_pc[g] = gen_pc[g]; p->gen_k[g] = gen_k[g]; }
+  p->n_gen = n_gen;
+  free(p->bank); p->bank = p->kbank; p->n_bank = p->n_kbank; p->kbank = NULL; p->n_kbank = 0;
+  free(p->ksrc); p->ksrc = NULL; p->n_ksrc = 0;
+  p->hist_id = p->khist.id; p->hist_nseg = p->khist.nseg; p->hist_ncoll = p->khist.ncoll; p->n_hist = p->khist.n;
+  memset(&p->khist, 0, sizeof p->khist);
+  const uint32_t n_active = n_gen - n_inactive;
   double sum = 0.0;
   for (uint32_t g = n_inactive; g < n_gen; g++) sum = sum + p->gen_k[g];
   p->k_mean = n_active ? sum / (double)n_active : 0.0;
@@ -686,6 +711,38 @@ int orc_run_k_eigenvalue(orc_problem *p, uint64_t n, uint32_t n_inactive, uint32
   p->k_std = n_active > 1 ? sqrt((var / (double)(n_active - 1)) / (double)n_active) : 0.0;
   p->ran = 1;
   return ORC_OK;
+}
+
+int orc_run_k_eigenvalue(orc_problem *p, uint64_t n, uint32_t n_inactive, uint32_t n_active, uint64_t seed) {
+  if (!p || n == 0 || (uint64_t)n_inactive + n_active == 0 || (uint64_t)n_inactive + n_active > 65535) return ORC_EINVAL;
+  uint32_t n_gen = n_inactive + n_active;
+  int rc = orc_k_begin(p, 0, n, n_gen, seed); if (rc) return rc;
+  uint64_t *gn = (uint64_t *)calloc(n_gen, 8), *gm = (uint64_t *)calloc(n_gen, 8);
+  int64_t *gp = (int64_t *)calloc(n_gen, 8), *gpc = (int64_t *)calloc(n_gen, 8);
+  double *gk = (double *)calloc(n_gen, 8);
+  double k_prev = 1.0;
+  uint32_t done = 0;
+  for (uint32_t g = 0; g < n_gen && !rc; g++) {
+    int64_t sums[4];
+    int last = (g + 1 == n_gen);
+    rc = orc_k_generation(p, g, g >= n_inactive, k_prev, last, sums);
+    if (rc) break;
+    double k = ((double)sums[0] * (1.0 / p->scale)) / (double)sums[2];       /* D2 */
+    gn[g] = (uint64_t)sums[2]; gm[g] = (uint64_t)sums[3]; gp[g] = sums[0]; gpc[g] = sums[1]; gk[g] = k;
+    done = g + 1;
+    if (sums[3] == 0) { rc = ORC_ESTATE; break; }
+    if (last) break;
+    /* population control: m = floor(N/M + xi) copies per site, unit weights */
+    double pr = (double)n / (double)sums[3];
+    uint64_t n_next = 0;
+    rc = orc_k_popctrl(p, g + 1, pr, &n_next);
+    k_prev = k;
+    if (!rc && n_next == 0) rc = ORC_ESTATE;
+  }
+  if (!rc) rc = orc_k_end(p, n_gen, n_inactive, gn, gm, gp, gpc, gk);
+  else { for (uint32_t g = 0; g < done; g++) { p->gen_n[g] = gn[g]; p->gen_m[g] = gm[g]; p->gen_p[g] = gp[g]; p->gen_pc[g] = gpc[g]; p->gen_k[g] = gk[g]; } p->n_gen = done; }
+  free(gn); free(gm); free(gp); free(gpc); free(gk);
+  return rc;
 }
 
 int orc_tally_sizes(const orc_problem *p, orc_sizes *o) {

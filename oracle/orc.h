@@ -110,6 +110,13 @@ typedef struct orc_problem orc_problem;
 int orc_init_problem(const orc_geometry *, const orc_materials *, const orc_xs_tables *, orc_problem **out);
 int orc_run_fixed_source(orc_problem *, uint64_t n_particles, uint64_t seed);
 int orc_run_k_eigenvalue(orc_problem *, uint64_t n_particles, uint32_t n_inactive, uint32_t n_active, uint64_t seed);
+/* one share of a run split over several processes by contiguous id ranges */
+int orc_run_fixed_source_range(orc_problem *, uint64_t first_id, uint64_t n_particles, uint64_t seed);
+int orc_k_begin(orc_problem *, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed);
+int orc_k_generation(orc_problem *, uint32_t gen, int active, double k_prev, int keep_hist, int64_t sums[4]); /* P, Pc, N_local, M_local */
+int orc_k_popctrl(orc_problem *, uint32_t gen_next, double pr, uint64_t *n_next);
+int orc_k_end(orc_problem *, uint32_t n_gen, uint32_t n_inactive, const uint64_t *gen_n, const uint64_t *gen_m, const int64_t *gen_p,
+              const int64_t *gen_pc, const double *gen_k);
 int orc_tally_sizes(const orc_problem *, orc_sizes *out);
 int orc_read_tallies(const orc_problem *, orc_tallies *out);
 void orc_free_problem(orc_problem *);

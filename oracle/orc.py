@@ -78,6 +78,11 @@ def lib():
         L.orc_init_problem.argtypes = [C.POINTER(Geometry), C.POINTER(Materials), C.POINTER(XsTables), C.POINTER(C.c_void_p)]
         L.orc_run_fixed_source.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
         L.orc_run_k_eigenvalue.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint64]
+        L.orc_run_fixed_source_range.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64]
+        L.orc_k_begin.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64]
+        L.orc_k_generation.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_double, C.c_int, C.POINTER(C.c_int64)]
+        L.orc_k_popctrl.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.POINTER(C.c_uint64)]
+        L.orc_k_end.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.orc_tally_sizes.argtypes = [C.c_void_p, C.POINTER(Sizes)]
         L.orc_read_tallies.argtypes = [C.c_void_p, C.POINTER(Tallies)]
         L.orc_free_problem.argtypes = [C.c_void_p]
@@ -153,6 +158,45 @@ class Oracle:
                                             p.n_active if n_active is None else n_active, seed)
         if rc:
             raise RuntimeError(f"oracle run failed: {rc}")
+        return self.read()
+
+    def run_fixed_source_range(self, first_id, n, seed):
+        rc = lib().orc_run_fixed_source_range(self.h, first_id, n, seed)
+        if rc:
+            raise RuntimeError(f"oracle run failed: {rc}")
+        return self.read()
+
+    # D2 in steps: the same four calls the CUDA library offers, so that the multi-process driver can be tested on CPU
+    def k_begin(self, first_id, n_local, n_gen, seed):
+        rc = lib().orc_k_begin(self.h, first_id, n_local, n_gen, seed)
+        if rc:
+            raise RuntimeError(f"orc_k_begin failed: {rc}")
+
+    def k_generation(self, gen, active, k_prev, last):
+        sums = (C.c_int64 * 4)()
+        rc = lib().orc_k_generation(self.h, gen, int(active), k_prev, int(last), sums)
+        if rc:
+            raise RuntimeError(f"orc_k_generation failed: {rc}")
+        return list(sums)
+
+    def k_population_control(self, gen_next, pr):
+        n = C.c_uint64()
+        rc = lib().orc_k_popctrl(self.h, gen_next, pr, C.byref(n))
+        if rc:
+            raise RuntimeError(f"orc_k_popctrl failed: {rc}")
+        return n.value
+
+    def k_end(self, n_inactive, gen_n, gen_m, gen_p, gen_pc, gen_k):
+        a = [np.ascontiguousarray(gen_n, np.uint64), np.ascontiguousarray(gen_m, np.uint64), np.ascontiguousarray(gen_p, np.int64),
+             np.ascontiguousarray(gen_pc, np.int64), np.ascontiguousarray(gen_k, np.float64)]
+        rc = lib().orc_k_end(self.h, len(a[0]), n_inactive, *[x.ctypes.data for x in a])
+        if rc:
+            raise RuntimeError(f"orc_k_end failed: {rc}")
+
+    def scale(self):
+        return float(2 ** int(self.problem.geometry["tally_scale_log2"]))
+
+    def read_tallies(self, history=True, bank=True):
         return self.read()
 
     def read(self):

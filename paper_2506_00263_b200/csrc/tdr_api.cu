@@ -10,6 +10,8 @@
 #include "tdr_stack.cuh"
 #include "tdr_split.cuh"
 #include "tdr_async.cuh"
+#include "tdr_pstash.cuh"
+#include "tdr_cstash.cuh"
 
 static thread_local char g_err[512] = "";
 static int fail(int code, const char *fmt, ...) {
@@ -40,6 +42,9 @@ struct tdr_problem {
   u64 id_offset = 0;                       // fixed source: ids id_offset .. id_offset + n - 1
   int drain_below = 65536;                 // stack scheme, k-mode: population below which the tail is drained in one launch
   int sync_every = 6;                      // stack scheme: remap iterations launched per counter read-back
+  int stash = -1;                          // async scheme: -1 = auto (multigroup: 2, continuous energy: 0); 0 = index stash per warp (slot numbers; state SoA in global memory), 1 = whole-particle stash per warp, 2 = whole-particle stash shared by the CTA
+  int pool_slots = 64;                     // particle stash: particle slots per warp
+  int ps_threads = PS_THREADS;             // particle stash: threads per CTA
   u64 bank_cap_opt = 0;                    // tests: fission-bank capacity in sites (0 = 2.5 n + 4096)
   u64 arena_links_opt = 0;                 // tests: global link arena of the asynchronous scheme (0 = 2 W/32 + 4096)
   // workspace
@@ -48,7 +53,7 @@ struct tdr_problem {
   Soa soa; u32 *stacks[EV_COUNT]; u64 *ctr; DevOut out; tdr_site *bank, *srcbank, *sec;
   u64 bank_cap = 0, src_cap = 0, sec_cap = 0, hist_cap = 0, W = 0;
   u64 *hist_id; u32 *hist_nseg, *hist_ncoll;
-  AsyncMem am;
+  AsyncMem am; PsMem pm;
   // results on host
   bool ran = false;
   std::vector<u64> gen_n, gen_m; std::vector<i64> gen_p, gen_pc; std::vector<double> gen_k;
@@ -56,6 +61,8 @@ struct tdr_problem {
   tdr_diag diag;
   int num_sms = 148;
   u64 *h_ctr = nullptr;                    // pinned readback
+  // D2 in steps
+  u64 k_first = 0, k_nsrc = 0, k_seed = 0, k_last_bank = 0; u32 k_ngen = 0; bool k_keep = false; double k_clock_ms = 0;
   std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
 };
 
@@ -236,6 +243,9 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "idle_timeout_s") { int n = atoi(value); if (n < 1 || n > 3600) return fail(TDR_EINVAL, "idle_timeout_s in [1,3600]"); p->idle_timeout_s = n; }
   else if (k == "id_offset") p->id_offset = strtoull(value, nullptr, 10);
   else if (k == "drain_below") { int n = atoi(value); if (n < 0) return fail(TDR_EINVAL, "drain_below >= 0"); p->drain_below = n; }
+  else if (k == "stash") { if (v == "auto") p->stash = -1; else if (v == "index") p->stash = 0; else if (v == "particle") p->stash = 1; else if (v == "shared") p->stash = 2; else return fail(TDR_EINVAL, "stash must be auto|index|particle|shared"); }
+  else if (k == "pool_slots") { int n = atoi(value); if (n < 32 || n > PS_RING || n % 8) return fail(TDR_EINVAL, "pool_slots: a multiple of 8 in [32,%d]", PS_RING); p->pool_slots = n; }
+  else if (k == "ps_threads") { int n = atoi(value); if (n < 32 || n > PS_THREADS || n % 32) return fail(TDR_EINVAL, "ps_threads: a multiple of 32 in [32,%d]", PS_THREADS); p->ps_threads = n; }
   else if (k == "bank_cap") p->bank_cap_opt = strtoull(value, nullptr, 10);
   else if (k == "arena_links") p->arena_links_opt = strtoull(value, nullptr, 10);
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
@@ -277,10 +287,11 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
   u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
   AsyncMem am; async_layout(c, W, sec_cap, p->arena_links_opt, am);
+  PsMem pm; pstash_layout(c, W, p->arena_links_opt, pm);
   if (assign) {
     p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
     p->bank = bank; p->srcbank = src; p->sec = sec; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
-    p->hist_cap = hist_cap; p->hist_id = hid; p->hist_nseg = hs; p->hist_ncoll = hc; p->am = am;
+    p->hist_cap = hist_cap; p->hist_id = hid; p->hist_nseg = hs; p->hist_ncoll = hc; p->am = am; p->pm = pm;
   }
   return (c.off + 255) & ~255ull;
 }
@@ -492,6 +503,82 @@ static int run_async(tdr_problem *p, DevRun R) {
   return 0;
 }
 
+// ---------------------------------------------------------------------------------- asynchronous scheme, whole-particle stash
+template <bool CE, int MODE>
+static int launch_pstash(tdr_problem *p, const DevRun &R, size_t smem, int threads) {
+  auto kernel = k_pstash<CE, MODE>;
+  CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int bps = p->blocks_per_sm;
+  if (bps <= 0) { if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, threads, smem) != cudaSuccess || bps < 1) return fail(TDR_EINVAL, "particle stash: %zu bytes of shared memory per CTA do not fit an SM (fewer pool_slots or ps_threads)", smem); }
+  KTimer t(p, true);
+  kernel<<<p->num_sms * bps, threads, smem, p->stream>>>(p->dp, p->out, R, p->pm, p->pool_slots, (u64)p->idle_timeout_s * 1000000000ull);
+  return 0;
+}
+
+template <bool CE>
+static int run_pstash(tdr_problem *p, DevRun R) {
+  cudaStream_t st = p->stream;
+  const int threads = p->ps_threads;
+  const size_t smem = smem_bytes(p) + (threads / 32) * PsPool<CE>::bytes(p->pool_slots);
+  if (smem > 227 * 1024) return fail(TDR_EINVAL, "particle stash needs %zu bytes of shared memory per CTA (limit 227 KB)", smem);
+  R.defer_death = 1; R.outstanding = p->ctr + C_PENDING; R.starved = p->ctr + C_STARVED; R.W = p->W;
+  k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull);
+  LAUNCH_CHECK();
+  int rc = p->split == 2 ? launch_pstash<CE, 2>(p, R, smem, threads) : launch_pstash<CE, 0>(p, R, smem, threads);
+  if (rc) return rc;
+  LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
+  u64 *h = p->h_ctr;
+  CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(h + 40, p->pm.ctr, PC_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  p->diag.spills += h[40 + PC_SPILLS]; p->diag.fetches += h[40 + PC_FETCHES]; p->diag.make_work_calls += h[40 + PC_EV_BIRTH];
+  p->diag.events[0] += h[40 + PC_LN_BIRTH]; p->diag.events[2] += h[40 + PC_LN_MOVE]; p->diag.events[4] += h[40 + PC_LN_COLLIDE];
+  p->diag.events[1] += h[40 + PC_EV_MOVE] + h[40 + PC_EV_COLLIDE] + h[40 + PC_EV_BIRTH];     // warp-level events (32 lanes each at best)
+  if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
+  if (!R.kmode && (h[C_PENDING] != 0 || h[40 + PC_GWORK] != 0))
+    return fail(TDR_ESTATE, "particle stash left %llu particles outstanding, %llu links queued", h[C_PENDING], h[40 + PC_GWORK]);
+  return 0;
+}
+
+// ---------------------------------------------------------------------------------- asynchronous scheme, stash shared by the CTA
+template <bool CE, int MODE>
+static int launch_cstash(tdr_problem *p, const DevRun &R, size_t smem, int threads, int ns) {
+  auto kernel = k_cstash<CE, MODE>;
+  CK(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int bps = p->blocks_per_sm;
+  if (bps <= 0) { if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, threads, smem) != cudaSuccess || bps < 1) return fail(TDR_EINVAL, "shared stash: %zu bytes of shared memory per CTA do not fit an SM (fewer pool_slots or ps_threads)", smem); }
+  KTimer t(p, true);
+  kernel<<<p->num_sms * bps, threads, smem, p->stream>>>(p->dp, p->out, R, p->pm, ns, (u64)p->idle_timeout_s * 1000000000ull);
+  return 0;
+}
+
+template <bool CE>
+static int run_cstash(tdr_problem *p, DevRun R) {
+  cudaStream_t st = p->stream;
+  const int threads = p->ps_threads <= CS_THREADS ? p->ps_threads : CS_THREADS;
+  const int ns = p->pool_slots * (threads / 32);
+  if (ns > 32768) return fail(TDR_EINVAL, "shared stash: more than 32768 slots per CTA");
+  const size_t smem = smem_bytes(p) + CsPool<CE>::bytes(ns);
+  if (smem > 227 * 1024) return fail(TDR_EINVAL, "shared stash needs %zu bytes of shared memory per CTA (limit 227 KB)", smem);
+  R.defer_death = 1; R.outstanding = p->ctr + C_PENDING; R.starved = p->ctr + C_STARVED; R.W = p->W;
+  k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull);
+  LAUNCH_CHECK();
+  int rc = p->split == 2 ? launch_cstash<CE, 2>(p, R, smem, threads, ns) : launch_cstash<CE, 0>(p, R, smem, threads, ns);
+  if (rc) return rc;
+  LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
+  u64 *h = p->h_ctr;
+  CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(h + 40, p->pm.ctr, PC_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  p->diag.spills += h[40 + PC_SPILLS]; p->diag.fetches += h[40 + PC_FETCHES]; p->diag.make_work_calls += h[40 + PC_EV_BIRTH];
+  p->diag.events[0] += h[40 + PC_LN_BIRTH]; p->diag.events[2] += h[40 + PC_LN_MOVE]; p->diag.events[4] += h[40 + PC_LN_COLLIDE];
+  p->diag.events[1] += h[40 + PC_EV_MOVE] + h[40 + PC_EV_COLLIDE] + h[40 + PC_EV_BIRTH];
+  if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
+  if (!R.kmode && (h[C_PENDING] != 0 || h[40 + PC_GWORK] != 0))
+    return fail(TDR_ESTATE, "shared stash left %llu particles outstanding, %llu links queued", h[C_PENDING], h[40 + PC_GWORK]);
+  return 0;
+}
+
 // one generation (or the whole fixed-source run) under the selected scheme
 static int run_generation(tdr_problem *p, DevRun &R) {
   cudaStream_t st = p->stream;
@@ -503,7 +590,12 @@ static int run_generation(tdr_problem *p, DevRun &R) {
   R.bank = p->bank; R.bank_cap = p->bank_cap;
   R.hist_id = p->hist_id; R.hist_nseg = p->hist_nseg; R.hist_ncoll = p->hist_ncoll;
   if (p->scheme == 0) return p->ce ? run_stack<true>(p, R) : run_stack<false>(p, R);
-  return p->ce ? run_async<true>(p, R) : run_async<false>(p, R);
+  // auto: the shared particle stash where the path is instruction bound (multigroup); the index stash where it is bound by
+  // cross-section gathers and wants the L1 that a particle stash would take (continuous energy) — DESIGN.md section 6
+  const int stash = p->stash >= 0 ? p->stash : (p->ce ? 0 : 2);
+  if (stash == 2 && p->split != 1) return p->ce ? run_cstash<true>(p, R) : run_cstash<false>(p, R);
+  if (stash == 1 && p->split != 1) return p->ce ? run_pstash<true>(p, R) : run_pstash<false>(p, R);
+  return p->ce ? run_async<true>(p, R) : run_async<false>(p, R);      // index stash; the five-event decomposition always
 }
 
 static int begin_run(tdr_problem *p, u64 n) {
@@ -547,42 +639,64 @@ int tdr_run_fixed_source(tdr_problem *p, uint64_t n, uint64_t seed) {
   return TDR_OK;
 }
 
-int tdr_run_k_eigenvalue(tdr_problem *p, uint64_t n, uint32_t n_inactive, uint32_t n_active, uint64_t seed) {
-  if ((u64)n_inactive + n_active == 0 || (u64)n_inactive + n_active > 65535) return fail(TDR_EINVAL, "bad generation counts");
-  int rc = begin_run(p, n); if (rc) return rc;
+// ---------------------------------------------------------------------------------- D2 in steps (one problem on several GPUs)
+int tdr_k_begin(tdr_problem *p, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed) {
+  if (n_gen == 0 || n_gen > 65535) return fail(TDR_EINVAL, "bad generation counts");
+  int rc = begin_run(p, n_local ? n_local : 1); if (rc) return rc;
+  p->k_first = first_id; p->k_nsrc = n_local; p->k_seed = seed; p->k_ngen = n_gen; p->k_last_bank = 0;
+  p->k_keep = p->keep_history < 0 ? n_local <= 2000000 : p->keep_history != 0;
+  p->k_clock_ms = 0.0;
+  return TDR_OK;
+}
+
+int tdr_k_generation(tdr_problem *p, uint32_t gen, int active, double k_prev, int last, int64_t sums[4]) {
+  if (!p || !sums || !p->ws) return fail(TDR_EINVAL, "bad argument");
   RunClock clk(p->stream);
   cudaStream_t st = p->stream;
-  const u32 n_gen = n_inactive + n_active;
-  u64 n_src = n; double k_prev = 1.0;
-  bool keep = p->keep_history < 0 ? n <= 2000000 : p->keep_history != 0;
-  for (u32 g = 0; g < n_gen; g++) {
-    DevRun R; memset(&R, 0, sizeof R);
-    R.seed = seed; R.gen = g; R.kmode = 1; R.active = g >= n_inactive; R.k_prev = k_prev;
-    R.src_sites = g > 0; R.sites = p->srcbank; R.src_total = n_src;
-    bool last = g + 1 == n_gen;
-    R.hist_cap = (keep && last) ? p->hist_cap : 0;
-    if ((rc = run_generation(p, R))) return rc;
-    CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(p->h_ctr + 16, p->out.PPc, 16, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    u64 M = p->h_ctr[C_BANK]; i64 P = (i64)p->h_ctr[16], Pc = (i64)p->h_ctr[17];
-    if (M > p->bank_cap) return fail(TDR_ECAPACITY, "fission bank overflow");
-    double k = ((double)P * (1.0 / p->dp.scale)) / (double)n_src;                    // D2
-    p->gen_n.push_back(n_src); p->gen_m.push_back(M); p->gen_p.push_back(P); p->gen_pc.push_back(Pc); p->gen_k.push_back(k);
-    if (M == 0) return fail(TDR_ESTATE, "fission bank empty in generation %u", g);
-    if (last) { p->n_bank = M; p->n_hist = R.hist_cap ? p->h_ctr[C_HIST] : 0; break; }
-    double pr = (double)n / (double)M;
-    CK(cudaMemsetAsync(p->ctr + C_NEXT_BANK, 0, 8, st));
-    k_popctrl<<<p->num_sms * 4, 256, 0, st>>>(p->bank, M, p->srcbank, p->src_cap, p->ctr + C_NEXT_BANK, seed, g + 1, pr, p->out.err);
-    LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.events[6] += M;
-    CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    if ((rc = check_dev_err(p, (int)p->h_ctr[C_COUNT - 1]))) return rc;
-    n_src = p->h_ctr[C_NEXT_BANK]; k_prev = k;
-    if (n_src == 0) return fail(TDR_ESTATE, "population died out");
-  }
-  p->diag.gpu_ms = clk.stop();
+  DevRun R; memset(&R, 0, sizeof R);
+  R.seed = p->k_seed; R.gen = gen; R.kmode = 1; R.active = active != 0; R.k_prev = k_prev;
+  R.src_sites = gen > 0; R.sites = p->srcbank; R.src_total = p->k_nsrc; R.id_offset = p->k_first;
+  R.hist_cap = (p->k_keep && last) ? p->hist_cap : 0;
+  int rc;
+  if (p->k_nsrc > 0) { if ((rc = run_generation(p, R))) return rc; }
+  else { CK(cudaMemsetAsync(p->ctr, 0, C_COUNT * 8, st)); CK(cudaMemsetAsync(p->out.PPc, 0, 16, st)); }     // a rank without a share
+  CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(p->h_ctr + 16, p->out.PPc, 16, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const u64 M = p->h_ctr[C_BANK];
+  if (M > p->bank_cap) return fail(TDR_ECAPACITY, "fission bank overflow");
+  sums[0] = (i64)p->h_ctr[16]; sums[1] = (i64)p->h_ctr[17]; sums[2] = (i64)p->k_nsrc; sums[3] = (i64)M;
+  p->k_last_bank = M;
+  if (last) { p->n_bank = M; p->n_hist = R.hist_cap ? p->h_ctr[C_HIST] : 0; }
+  p->k_clock_ms += clk.stop();
+  return TDR_OK;
+}
+
+int tdr_k_population_control(tdr_problem *p, uint32_t gen_next, double pr, uint64_t *n_next) {
+  if (!p || !n_next || !p->ws) return fail(TDR_EINVAL, "bad argument");
+  RunClock clk(p->stream);
+  cudaStream_t st = p->stream;
+  const u64 M = p->k_last_bank;
+  CK(cudaMemsetAsync(p->ctr + C_NEXT_BANK, 0, 8, st));
+  if (M) { k_popctrl<<<p->num_sms * 4, 256, 0, st>>>(p->bank, M, p->srcbank, p->src_cap, p->ctr + C_NEXT_BANK, p->k_seed, gen_next, pr, p->out.err); LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.events[6] += M; }
+  CK(cudaMemcpyAsync(p->h_ctr, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  int rc;
+  if ((rc = check_dev_err(p, (int)p->h_ctr[C_COUNT - 1]))) return rc;
+  p->k_nsrc = p->h_ctr[C_NEXT_BANK];
+  *n_next = p->k_nsrc;
+  p->k_clock_ms += clk.stop();
+  return TDR_OK;
+}
+
+int tdr_k_end(tdr_problem *p, uint32_t n_gen, uint32_t n_inactive, const uint64_t *gen_n, const uint64_t *gen_m, const int64_t *gen_p,
+              const int64_t *gen_pc, const double *gen_k) {
+  if (!p || n_gen == 0 || n_inactive > n_gen || !gen_n || !gen_m || !gen_p || !gen_pc || !gen_k) return fail(TDR_EINVAL, "bad argument");
+  p->gen_n.assign(gen_n, gen_n + n_gen); p->gen_m.assign(gen_m, gen_m + n_gen); p->gen_p.assign(gen_p, gen_p + n_gen);
+  p->gen_pc.assign(gen_pc, gen_pc + n_gen); p->gen_k.assign(gen_k, gen_k + n_gen);
+  p->diag.gpu_ms = p->k_clock_ms;
   collect_kernel_times(p);
+  const u32 n_active = n_gen - n_inactive;
   double sum = 0.0;
   for (u32 g = n_inactive; g < n_gen; g++) sum = sum + p->gen_k[g];
   p->k_mean = n_active ? sum / (double)n_active : 0.0;
@@ -591,6 +705,31 @@ int tdr_run_k_eigenvalue(tdr_problem *p, uint64_t n, uint32_t n_inactive, uint32
   p->k_std = n_active > 1 ? sqrt((var / (double)(n_active - 1)) / (double)n_active) : 0.0;
   p->ran = true;
   return TDR_OK;
+}
+
+// D2 on one GPU: the loop over the steps above with a single share
+int tdr_run_k_eigenvalue(tdr_problem *p, uint64_t n, uint32_t n_inactive, uint32_t n_active, uint64_t seed) {
+  if ((u64)n_inactive + n_active == 0 || (u64)n_inactive + n_active > 65535) return fail(TDR_EINVAL, "bad generation counts");
+  if (n == 0) return fail(TDR_EINVAL, "bad argument");
+  const u32 n_gen = n_inactive + n_active;
+  int rc = tdr_k_begin(p, 0, n, n_gen, seed); if (rc) return rc;
+  std::vector<u64> gn, gm; std::vector<i64> gp, gpc; std::vector<double> gk;
+  double k_prev = 1.0;
+  for (u32 g = 0; g < n_gen; g++) {
+    i64 sums[4];
+    const bool last = g + 1 == n_gen;
+    if ((rc = tdr_k_generation(p, g, g >= n_inactive, k_prev, last, (int64_t *)sums))) return rc;
+    const double k = ((double)sums[0] * (1.0 / p->dp.scale)) / (double)sums[2];                    // D2
+    gn.push_back((u64)sums[2]); gm.push_back((u64)sums[3]); gp.push_back(sums[0]); gpc.push_back(sums[1]); gk.push_back(k);
+    if (sums[3] == 0) return fail(TDR_ESTATE, "fission bank empty in generation %u", g);
+    if (last) break;
+    const double pr = (double)n / (double)sums[3];
+    u64 n_next = 0;
+    if ((rc = tdr_k_population_control(p, g + 1, pr, (uint64_t *)&n_next))) return rc;
+    k_prev = k;
+    if (n_next == 0) return fail(TDR_ESTATE, "population died out");
+  }
+  return tdr_k_end(p, n_gen, n_inactive, (const uint64_t *)gn.data(), (const uint64_t *)gm.data(), (const int64_t *)gp.data(), (const int64_t *)gpc.data(), gk.data());
 }
 
 int tdr_tally_sizes(const tdr_problem *p, tdr_sizes *o) {

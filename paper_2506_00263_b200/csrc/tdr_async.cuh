@@ -41,7 +41,8 @@ __device__ __forceinline__ u64 ld_vol(const u64 *p) { return *(const volatile u6
 __device__ __forceinline__ u64 global_ns() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
 
 // ---------------------------------------------------------------------------------- global queues (lane 0 only)
-__device__ __noinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine) {
+template <class LinkT>
+__device__ __noinline__ void q_deposit(LinkT *links, u64 *qs, u32 i, u64 mine) {
   for (;;) {
     u64 cur = atomicExch(&qs[i], NULLQ);                         // claim whatever is there
     if (cur != NULLQ) {                                          // merge privately: cur ++ mine
@@ -56,7 +57,8 @@ __device__ __noinline__ void q_deposit(GLink *links, u64 *qs, u32 i, u64 mine) {
 }
 
 // A claimed queue looks like an empty one, so `rounds` full scans are made before the set is taken to be empty.
-__device__ __noinline__ u32 q_pop(GLink *links, u64 *qs, u32 start, u32 rounds) {
+template <class LinkT>
+__device__ __noinline__ u32 q_pop(LinkT *links, u64 *qs, u32 start, u32 rounds) {
   for (u32 a = 0; a < AQ * rounds; a++) {
     u32 i = (start + a) % AQ;
     if (ld_vol(&qs[i]) == NULLQ) continue;

@@ -75,7 +75,17 @@ struct Part {
 // ---------------------------------------------------------------------------------- R1 Philox4x32-10
 struct Blk { u32 w0, w1, w2, w3; };
 
-__device__ __forceinline__ Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {
+#ifdef TDR_PHILOX_CALL
+#define TDR_PHILOX_ATTR __noinline__
+#else
+#define TDR_PHILOX_ATTR __forceinline__
+#endif
+#ifdef TDR_COLD_CALL
+#define TDR_COLD __noinline__
+#else
+#define TDR_COLD __forceinline__
+#endif
+__device__ TDR_PHILOX_ATTR Blk philox(u32 c0, u32 c1, u32 c2, u32 c3, u32 k0, u32 k1) {
 #pragma unroll
   for (int r = 0; r < 10; r++) {
     u32 h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
@@ -132,6 +142,7 @@ __device__ __forceinline__ i64 fixp(double v, double scale) { return __double2ll
 
 // ---------------------------------------------------------------------------------- B2 / B3 / T6 samplers
 __device__ __forceinline__ int iso_dir(u64 seed, u64 id, u32 gen, u32 seg, double &u, double &v, double &w) {
+#pragma unroll 1
   for (u32 a = 0; a < MAX_ATTEMPT; a++) {
     Blk b = rng_block(seed, id, gen, seg, PUR_DIR, a);
     double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;
@@ -148,6 +159,7 @@ __device__ __forceinline__ int iso_dir(u64 seed, u64 id, u32 gen, u32 seg, doubl
 
 __device__ __forceinline__ double watt(u64 seed, u64 id, u32 gen, double a, double b) {
   double cos2 = 1.0;
+#pragma unroll 1
   for (u32 t = 0; t < MAX_ATTEMPT; t++) {
     Blk k = rng_block(seed, id, gen, 0, PUR_ENERGY, 4 + t);          // j = 8+2t, 9+2t
     double v1 = 2.0 * blk_even(k) - 1.0, v2 = 2.0 * blk_odd(k) - 1.0;
@@ -168,6 +180,7 @@ __device__ __forceinline__ void scatter_ce(u64 seed, u32 gen, Part &p, double A)
   p.E = p.E * (q / ((A + 1.0) * (A + 1.0)));
   double mul = (1.0 + A * mu) / sqrt(q);
   double cphi = 1.0, sphi = 0.0;
+#pragma unroll 1
   for (u32 t = 0; t < MAX_ATTEMPT; t++) {
     Blk b = rng_block(seed, p.id, gen, p.seg, PUR_DIR, t);
     double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;

@@ -215,7 +215,7 @@ __device__ __forceinline__ void record_death(BlockAcc *a, const DevRun &R, const
 }
 
 // the same bookkeeping for a whole link of dead particles (valid = lane holds one): warp-reduced, one atomic each
-__device__ __forceinline__ void record_deaths_warp(BlockAcc *a, const DevRun &R, bool valid, u64 id, u32 seg, u32 ncoll) {
+__device__ TDR_COLD void record_deaths_warp(BlockAcc *a, const DevRun &R, bool valid, u64 id, u32 seg, u32 ncoll) {
   const u32 lane = threadIdx.x & 31;
   const u32 m = __ballot_sync(FULL, valid);
   if (m == 0) return;
@@ -333,7 +333,7 @@ __device__ __forceinline__ void birth_common(const DevProb &P, const double *mg,
 }
 
 template <bool CE>
-__device__ __forceinline__ void birth_primary(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, u64 i) {
+__device__ TDR_COLD void birth_primary(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, u64 i) {
   p.id = i + R.id_offset; p.depth = 0;         // id_offset: this GPU's share of a source sharded by contiguous id ranges
   if (P.src_kind == 0) { p.x = P.src_lo[0]; p.y = P.src_lo[1]; p.z = P.src_lo[2]; }
   else {
@@ -350,7 +350,7 @@ __device__ __forceinline__ void birth_primary(const DevProb &P, const double *mg
 }
 
 template <bool CE>
-__device__ __forceinline__ void birth_site(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, const tdr_site &s) {
+__device__ TDR_COLD void birth_site(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, const tdr_site &s) {
   p.id = s.id; p.depth = s.depth; p.x = s.x; p.y = s.y; p.z = s.z;
   p.ix = s.ix; p.iy = s.iy; p.iz = s.iz; p.mx = s.mx; p.my = s.my; p.mz = s.mz; p.ring = s.ring;
   birth_common<CE>(P, mg, R, acc, p, s.src, true);

@@ -30,7 +30,7 @@ __device__ __forceinline__ void stack_push(u32 *stack, u64 *count, u32 value, bo
 }
 
 // warp-collective push of n sites per lane into the fission bank (k-mode) or the secondary ring (fixed source)
-__device__ __forceinline__ void push_children(const DevOut &O, const DevRun &R, BlockAcc *acc, const Part &p, int n, int src) {
+__device__ TDR_COLD void push_children(const DevOut &O, const DevRun &R, BlockAcc *acc, const Part &p, int n, int src) {
   u32 lane = threadIdx.x & 31;
   u32 total = __reduce_add_sync(FULL, (u32)n);
   if (total == 0) return;

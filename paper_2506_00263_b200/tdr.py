@@ -60,7 +60,7 @@ class tdr_diag(C.Structure):
 
 EXPORTS = ["tdr_init_problem", "tdr_set_option", "tdr_workspace_bytes", "tdr_bind_workspace", "tdr_run_fixed_source",
            "tdr_run_k_eigenvalue", "tdr_tally_sizes", "tdr_read_tallies", "tdr_read_diagnostics", "tdr_free_problem",
-           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw"]
+           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw", "tdr_k_begin", "tdr_k_generation", "tdr_k_population_control", "tdr_k_end"]
 
 _lib = None
 
@@ -69,7 +69,7 @@ def lib():
     """Load libtdr.so (building it in-tree if the sources are newer).  Raises if it cannot be loaded."""
     global _lib
     if _lib is None:
-        path = _build.build() if os.path.exists(_build.CSRC) else _build.LIB
+        path = os.environ.get("TDR_LIB") or (_build.build() if os.path.exists(_build.CSRC) else _build.LIB)   # TDR_LIB: a developer's trial build
         L = C.CDLL(path)
         L.tdr_init_problem.argtypes = [C.POINTER(tdr_geometry), C.POINTER(tdr_materials), C.POINTER(tdr_xs_tables), C.POINTER(C.c_void_p)]
         L.tdr_set_option.argtypes = [C.c_void_p, C.c_char_p, C.c_char_p]
@@ -77,6 +77,10 @@ def lib():
         L.tdr_bind_workspace.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
         L.tdr_run_fixed_source.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64]
         L.tdr_run_k_eigenvalue.argtypes = [C.c_void_p, C.c_uint64, C.c_uint32, C.c_uint32, C.c_uint64]
+        L.tdr_k_begin.argtypes = [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint64]
+        L.tdr_k_generation.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_double, C.c_int, C.POINTER(C.c_int64)]
+        L.tdr_k_population_control.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.POINTER(C.c_uint64)]
+        L.tdr_k_end.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.tdr_tally_sizes.argtypes = [C.c_void_p, C.POINTER(tdr_sizes)]
         L.tdr_read_tallies.argtypes = [C.c_void_p, C.POINTER(tdr_tallies)]
         L.tdr_read_diagnostics.argtypes = [C.c_void_p, C.POINTER(tdr_diag)]
@@ -157,6 +161,29 @@ class Problem:
     def run_k_eigenvalue(self, n_particles, n_inactive, n_active, seed):
         self._bind(n_particles)
         _check(lib().tdr_run_k_eigenvalue(self.h, n_particles, n_inactive, n_active, seed), "tdr_run_k_eigenvalue")
+
+    # D2 in steps (one problem on several GPUs; paper_2506_00263_b200.shard drives these)
+    def k_begin(self, first_id, n_local, n_gen, seed):
+        self._bind(max(n_local, 1))
+        _check(lib().tdr_k_begin(self.h, first_id, n_local, n_gen, seed), "tdr_k_begin")
+
+    def k_generation(self, gen, active, k_prev, last):
+        sums = (C.c_int64 * 4)()
+        _check(lib().tdr_k_generation(self.h, gen, int(active), k_prev, int(last), sums), "tdr_k_generation")
+        return list(sums)
+
+    def k_population_control(self, gen_next, pr):
+        n = C.c_uint64()
+        _check(lib().tdr_k_population_control(self.h, gen_next, pr, C.byref(n)), "tdr_k_population_control")
+        return n.value
+
+    def k_end(self, n_inactive, gen_n, gen_m, gen_p, gen_pc, gen_k):
+        a = [np.ascontiguousarray(gen_n, np.uint64), np.ascontiguousarray(gen_m, np.uint64), np.ascontiguousarray(gen_p, np.int64),
+             np.ascontiguousarray(gen_pc, np.int64), np.ascontiguousarray(gen_k, np.float64)]
+        _check(lib().tdr_k_end(self.h, len(a[0]), n_inactive, *[x.ctypes.data for x in a]), "tdr_k_end")
+
+    def scale(self):
+        return float(2 ** int(self.problem.geometry["tally_scale_log2"]))
 
     def run(self, n=None, n_inactive=None, n_active=None, seed=None):
         p = self.problem

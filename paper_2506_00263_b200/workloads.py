@@ -164,10 +164,11 @@ def two_region(kind="pin", n=200000, seed=1):
                        src_kind=1, src_lo=(-3 * h, -3 * h, 0.0), src_hi=(3 * h, 3 * h, 0.0))
         frac = pi * R * R / (4 * h * h)
     elif kind == "zones":
+        # three zones: pin R, bare moderator (a universe without rings), thin pin R2
         R2 = 0.30
-        geo = geometry([-h, h], [-h, h], [0.0, 1.0, 2.5], [0, 1], [((R,), (0, 1)), ((R2,), (0, 1))], [1] * 6,
-                       src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 2.5))
-        frac = (pi * R * R * 1.0 + pi * R2 * R2 * 1.5) / (4 * h * h * 2.5)
+        geo = geometry([-h, h], [-h, h], [0.0, 1.0, 2.5, 3.0], [0, 1, 2], [((R,), (0, 1)), ((), (1,)), ((R2,), (0, 1))], [1] * 6,
+                       src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 3.0))
+        frac = (pi * R * R * 1.0 + pi * R2 * R2 * 0.5) / (4 * h * h * 3.0)
     elif kind == "rings":
         R1 = 0.25
         geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((R1, R), (1, 0, 1))], [1, 1, 1, 1, 0, 0],

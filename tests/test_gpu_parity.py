@@ -126,7 +126,7 @@ def test_async_spill_and_fetch_through_the_global_queues(decomp):
     for p, kw in ((W.cfg1(n=300007, n_inactive=1, n_active=2), dict(lockstep=0, slots_per_warp=256)),
                   (W.cfg3(n=5003, n_ebins=100), dict(lockstep=0, slots_per_warp=256)),
                   (W.cfg2(n=200003, n_inactive=1, n_active=1), dict(lockstep=0 if decomp == "fused" else 1, stash_links=8, slots_per_warp=256))):
-        o, g, d = run_both(p, scheme="async", decomposition=decomp, force_spill=1, **kw)
+        o, g, d = run_both(p, scheme="async", stash="index", decomposition=decomp, force_spill=1, **kw)
         assert_same(o, g, f"spill stress {p.name}/{decomp}")
         assert d["fetches"] == d["spills"], d
         total += d["spills"]
@@ -171,12 +171,13 @@ def test_capacity_and_lost_particle_errors_are_reported():
         assert e.value.code == -4, e.value
         P.close()
     # asynchronous scheme: forced spills with a global link arena of 8 links -> TDR_ECAPACITY
-    P = tdr.Problem(W.cfg1(n=300007, n_inactive=1, n_active=1), scheme="async", decomposition="hybrid", force_spill=1, lockstep=0,
-                    slots_per_warp=256, arena_links=8)
-    with pytest.raises(tdr.TdrError) as e:
-        P.run()
-    assert e.value.code == -4, e.value
-    P.close()
+    for prob, kw in ((W.cfg1(n=300007, n_inactive=1, n_active=1), dict(stash="index", decomposition="hybrid", lockstep=0, slots_per_warp=256)),
+                     (W.cfg3(n=20011, n_ebins=100), dict(stash="particle")), (W.cfg3(n=20011, n_ebins=100), dict(stash="shared"))):
+        P = tdr.Problem(prob, scheme="async", force_spill=1, arena_links=8, **kw)
+        with pytest.raises(tdr.TdrError) as e:
+            P.run()
+        assert e.value.code == -4, (kw, e.value)
+        P.close()
     # a void with no boundary in reach: no finite distance -> TDR_ELOST (-5), as the oracle says too
     void = W.infinite_medium([0.0], [[0.0]], n=1000)
     for scheme in ("stack", "async"):
@@ -207,3 +208,61 @@ def test_results_do_not_depend_on_the_launch_configuration():
         g = P.run()
         P.close()
         assert_same(o, g, str(kw))
+
+
+# ------------------------------------------------------------------ the particle stashes
+PARTICLE_STASHES = [("particle", "fused"), ("particle", "hybrid"), ("shared", "fused"), ("shared", "hybrid")]
+
+
+@pytest.mark.parametrize("stash,decomp", PARTICLE_STASHES)
+@pytest.mark.parametrize("name", ["cfg0", "cfg1", "cfg2", "cfg3", "cfg4"])
+def test_particle_stash_parity_all_configs(name, stash, decomp):
+    """The asynchronous scheme with whole particles in the stash — per warp and shared by the CTA's warps
+     — on all five configs, with and without forced hand-over of secondaries through the global link queues."""
+    p = small_cases()[name]
+    for extra in ({}, {"force_spill": 1}, {"pool_slots": 32}):
+        o, g, d = run_both(p, scheme="async", stash=stash, decomposition=decomp, **extra)
+        assert_same(o, g, f"{name}/async/{stash}/{decomp}/{extra}")
+        assert d["spills"] == d["fetches"], d
+    if name == "cfg3":
+        assert d["spills"] > 0                               # fission secondaries really travelled through global links
+
+
+@pytest.mark.parametrize("stash", ["particle", "shared"])
+def test_particle_stash_edge_cases_and_full_size(stash):
+    for p in (W.cfg0(n=1), W.cfg0(n=31), W.cfg0(n=33), W.slab(1.3, 1.7, n=10007), W.cfg3(n=257, n_ebins=10000),
+              W.ce_slowing_down(A=16.0, n=2003), W.infinite_medium([1.0], [[0.5]], [0.34], [1.5], mode="fixed", n=300)):
+        o, g, _ = run_both(p, scheme="async", stash=stash, decomposition="hybrid")
+        assert_same(o, g, p.name)
+    for p in (W.cfg1(n_inactive=1, n_active=3), W.cfg3(n=1000000, n_ebins=100)):
+        o, g, _ = run_both(p, scheme="async", stash=stash, decomposition="hybrid")
+        assert_same(o, g, f"full-size {p.name}/{stash}")
+    from paper_2506_00263_b200 import tdr
+    for kw in (dict(ps_threads=128), dict(ps_threads=64, pool_slots=96), dict(blocks_per_sm=1)):
+        p = W.cfg1(n=100003, n_inactive=1, n_active=2)
+        o, g, _ = run_both(p, scheme="async", stash=stash, decomposition="hybrid", **kw)
+        assert_same(o, g, str(kw))
+
+
+# ------------------------------------------------------------------ one k-eigenvalue problem over several shares (SURVEY 8e)
+@pytest.mark.parametrize("scheme", ["stack", "async"])
+def test_k_eigenvalue_in_three_shares_equals_the_unsharded_oracle(scheme):
+    """Three shares of ONE problem driven in turn on one GPU (no kernel waits on another), exchanging only the four
+    per-generation sums: bit-identical to the oracle's un-sharded run — k per generation, tallies, totals, bank."""
+    from oracle import orc
+    from paper_2506_00263_b200 import shard, tdr
+    for p in (W.cfg1(n=30011, n_inactive=2, n_active=3), W.cfg4(n=20011, n_inactive=1, n_active=2)):
+        o = orc.run(p)
+        engines = [tdr.Problem(p, scheme=scheme) for _ in range(3)]
+        parts = shard.run_k_eigenvalue_shares(engines, [(r, 3) for r in range(3)], p.n_particles, p.n_inactive, p.n_active, p.seed)
+        for e in engines:
+            e.close()
+        m = shard.merge_local(parts)
+        for k in ("flux", "coll", "leak"):
+            assert np.array_equal(m[k], o[k]), (p.name, k)
+        assert m["totals"] == o["totals"], p.name
+        for k in ("gen_n", "gen_m", "gen_p", "gen_pc"):
+            assert np.array_equal(parts[2][k], o[k]), (p.name, k)
+        assert np.array_equal(parts[0]["gen_k"], o["gen_k"]) and parts[1]["k_mean"] == o["k_mean"]
+        bank = np.concatenate([x["bank"] for x in parts])
+        assert np.array_equal(np.sort(bank.view(np.dtype((np.void, 48)))), np.sort(o["bank"].view(np.dtype((np.void, 48)))))
