@@ -56,6 +56,13 @@ typedef struct tdr_geometry {
   int32_t src_index;
   double src_energy;
   int32_t tally_scale_log2;                  /* S: tallies are llrint(v * 2^S) summed in int64 */
+  /* time-dependent fixed source (readings TD1-TD6): time-mesh tally + census */
+  int32_t n_tbins;                           /* 0 = time-independent; <= 255 */
+  const double *t_edges;                     /* n_tbins+1 ascending: emission time ... census time */
+  /* implicit capture + weight roulette, the `closeout` of the paper's decomposed scheme (readings W1-W4);
+   * fixed-source runs only */
+  int32_t implicit_capture;                  /* 0 = analog (weights identically 1) */
+  double w_roulette, w_survive;              /* roulette below w_roulette; a survivor continues with w_survive */
 } tdr_geometry;
 
 typedef struct tdr_materials {
@@ -65,6 +72,7 @@ typedef struct tdr_materials {
   const int32_t *mat_nnuc;                   /* CE: n_mat */
   const int32_t *mat_nuc;                    /* CE: n_mat*TDR_MAX_NUC nuclide indices */
   const double *mat_dens;                    /* CE: n_mat*TDR_MAX_NUC atom densities (1/b-cm) */
+  const double *speed;                       /* MG, time-dependent runs only: speed of group g, [G] (CE: 1.3831592e6 cm/s x sqrt(E/eV)) */
 } tdr_materials;
 
 typedef struct tdr_xs_tables {               /* CE only; NULL for multigroup */
@@ -79,7 +87,7 @@ typedef struct tdr_site {                    /* fission-bank / source-bank recor
   double x, y, z;
   uint64_t id;
   int16_t ix, iy, iz, mx, my, mz;
-  uint8_t ring, src, depth, pad;
+  uint8_t ring, src, depth, it;              /* it: time bin (time-dependent fixed source), else 0 */
 } tdr_site;
 
 typedef struct tdr_sizes {
@@ -90,10 +98,10 @@ typedef struct tdr_sizes {
 } tdr_sizes;
 
 enum { TDR_T_NSEG = 0, TDR_T_NCOLL, TDR_T_NCROSS, TDR_T_NABS, TDR_T_NFIS, TDR_T_NLEAK, TDR_T_NBORN,
-       TDR_T_NDROPPED, TDR_T_NDIRFAIL, TDR_T_DIGEST, TDR_T_NSITES, TDR_T_COUNT = 12 };
+       TDR_T_NDROPPED, TDR_T_NDIRFAIL, TDR_T_DIGEST, TDR_T_NSITES, TDR_T_NCENSUS, TDR_T_NROULETTE, TDR_T_COUNT = 16 };
 
 typedef struct tdr_tallies {                 /* HOST buffers, caller-allocated; NULL = skip */
-  int64_t *flux, *coll;                      /* n_bins, bin = ((mz*ny_m+my)*nx_m+mx)*n_e + e */
+  int64_t *flux, *coll;                      /* n_bins, bin = (((it*nz_m+mz)*ny_m+my)*nx_m+mx)*n_e + e (it = 0 without a time mesh) */
   int64_t leak[6];
   uint64_t totals[TDR_T_COUNT];
   double k_mean, k_std;
@@ -157,6 +165,10 @@ const char *tdr_last_error(void);
 int tdr_dev_det_log(const double *x, double *out, uint64_t n, void *cuda_stream);
 int tdr_dev_draw(uint64_t seed, const uint64_t *id, uint32_t gen, uint32_t seg, uint32_t purpose, uint32_t j,
                  double *out, uint64_t n, void *cuda_stream);
+
+/* Measured ceilings for the roofline: what = 0 -> fp64 DFMA rate in TFLOP/s, 1 -> L2-resident copy bandwidth in
+ * GB/s (read + write bytes).  `value` is a HOST pointer; the call allocates and frees its own device scratch. */
+int tdr_measure_peak(int what, double *value, void *cuda_stream);
 
 #ifdef __cplusplus
 }

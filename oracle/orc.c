@@ -25,7 +25,7 @@ void orc_philox(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
 }
 
 enum { PUR_DIST = 0, PUR_SELECT = 1, PUR_ENERGY = 2, PUR_DIR = 3, PUR_MULT = 4, PUR_POS = 5,
-       PUR_POPCTRL = 6, PUR_IDDERIVE = 15 };
+       PUR_POPCTRL = 6, PUR_CLOSEOUT = 7, PUR_IDDERIVE = 15 };
 #define MAX_ATTEMPT 1024
 
 static void block(uint64_t seed, uint64_t id, uint32_t gen, uint32_t seg, uint32_t purpose,
@@ -176,8 +176,9 @@ int32_t orc_grid_index(const double *grid, int32_t n, double E) {
 typedef struct { uint64_t *id; uint32_t *nseg, *ncoll; size_t n, cap; } histvec;   /* per-history records */
 
 struct orc_problem {
-  int nx, ny, nz, bc[6], n_univ, mesh_n[3], by_group, n_e, S;
-  double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges;
+  int nx, ny, nz, bc[6], n_univ, mesh_n[3], by_group, n_e, S, n_t;           /* n_t: time bins (0 = time-independent) */
+  int implicit; double w_roulette, w_survive;                                /* W: implicit capture + roulette */
+  double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges, *t_edges, *speed;
   int32_t *cell_univ, *univ_nr, *univ_mat;
   int src_kind, src_dir_kind, src_energy_kind, src_index;
   double src_lo[3], src_hi[3], src_dir[3], src_energy, scale;
@@ -219,7 +220,7 @@ void orc_free_problem(orc_problem *p) {
   free_results(p);
   free(p->xp); free(p->yp); free(p->zp); free(p->cx); free(p->cy); free(p->univ_rad);
   for (int a = 0; a < 3; a++) free(p->mesh[a]);
-  free(p->e_edges); free(p->cell_univ); free(p->univ_nr); free(p->univ_mat);
+  free(p->e_edges); free(p->t_edges); free(p->speed); free(p->cell_univ); free(p->univ_nr); free(p->univ_mat);
   free(p->sig_t); free(p->sig_f); free(p->nu); free(p->sst); free(p->sig_c); free(p->scdf);
   free(p->chicdf); free(p->nusigf); free(p->mat_nnuc); free(p->mat_nuc); free(p->mat_dens);
   free(p->grid); free(p->A); free(p->xs_s); free(p->xs_c); free(p->xs_f); free(p->nuc_nu);
@@ -260,7 +261,17 @@ int orc_init_problem(const orc_geometry *g, const orc_materials *m, const orc_xs
   p->src_index = g->src_index; p->src_energy = g->src_energy;
   memcpy(p->src_lo, g->src_lo, 24); memcpy(p->src_hi, g->src_hi, 24); memcpy(p->src_dir, g->src_dir, 24);
   p->S = g->tally_scale_log2; p->scale = ldexp(1.0, p->S);
-  p->n_bins = (uint64_t)p->mesh_n[0] * p->mesh_n[1] * p->mesh_n[2] * p->n_e;
+  p->implicit = g->implicit_capture != 0; p->w_roulette = g->w_roulette; p->w_survive = g->w_survive;     /* W */
+  if (p->implicit && !(p->w_roulette > 0.0 && p->w_survive >= p->w_roulette)) { orc_free_problem(p); return ORC_EINVAL; }
+  p->n_t = g->n_tbins;                                                  /* TD: time mesh */
+  if (p->n_t < 0 || p->n_t > 255) { orc_free_problem(p); return ORC_EINVAL; }
+  if (p->n_t > 0) {
+    if (!g->t_edges || (p->G > 0 && !m->speed)) { orc_free_problem(p); return ORC_EINVAL; }
+    p->t_edges = DUPD(g->t_edges, p->n_t + 1);
+    for (int k = 0; k < p->n_t; k++) if (!(p->t_edges[k] < p->t_edges[k + 1])) { orc_free_problem(p); return ORC_EINVAL; }
+    if (p->G > 0) p->speed = DUPD(m->speed, p->G);
+  }
+  p->n_bins = (uint64_t)(p->n_t > 0 ? p->n_t : 1) * p->mesh_n[0] * p->mesh_n[1] * p->mesh_n[2] * p->n_e;
   if (p->G > 0) {                                                    /* X1 */
     int G = p->G, M = p->n_mat;
     p->sig_t = DUPD(m->sig_t, M * G); p->sig_f = DUPD(m->sig_f, M * G); p->nu = DUPD(m->nu, M * G);
@@ -294,8 +305,8 @@ int orc_init_problem(const orc_geometry *g, const orc_materials *m, const orc_xs
 
 /* ------------------------------------------------------------------ particle + per-thread context */
 typedef struct {
-  double x, y, z, u, v, w, E;
-  int g, ix, iy, iz, ring, mx, my, mz, depth;
+  double x, y, z, u, v, w, E, t, wgt;
+  int g, ix, iy, iz, ring, mx, my, mz, depth, it;
   uint64_t id; uint32_t seg, ncoll;
 } part;
 
@@ -307,7 +318,7 @@ typedef struct {
   int64_t *flux, *coll, leak[6];
   __int128 P, Pc;
   uint64_t tot[ORC_T_COUNT];
-  sitevec bank, stack;
+  sitevec bank, stack; double *stack_t, *stack_w; size_t stack_t_cap;     /* time (TD5) and weight (W1) of secondary stack.v[i] */
   histvec hist; int keep_hist;
   int err;
 } ctx;
@@ -368,6 +379,8 @@ static void birth_common(ctx *c, part *q, int src, int from_site) {
 static void birth_primary(ctx *c, part *q, uint64_t i) {                /* i = source id (D1: first_id + index) */
   const orc_problem *p = c->p;
   q->id = i; q->depth = 0;
+  q->it = 0; q->t = p->n_t > 0 ? p->t_edges[0] : 0.0;                   /* TD5: emitted at the first time edge */
+  q->wgt = 1.0;                                                         /* W1 */
   double pos[3];
   for (int a = 0; a < 3; a++) {
     if (p->src_kind == 0) pos[a] = p->src_lo[a];
@@ -382,8 +395,8 @@ static void birth_primary(ctx *c, part *q, uint64_t i) {                /* i = s
   birth_common(c, q, 0, 0);
 }
 
-static void birth_site(ctx *c, part *q, const orc_site *s) {
-  q->id = s->id; q->depth = s->depth;
+static void birth_site(ctx *c, part *q, const orc_site *s, double t, double wgt) {
+  q->id = s->id; q->depth = s->depth; q->t = t; q->it = s->it; q->wgt = wgt;
   q->x = s->x; q->y = s->y; q->z = s->z;
   q->ix = s->ix; q->iy = s->iy; q->iz = s->iz; q->mx = s->mx; q->my = s->my; q->mz = s->mz; q->ring = s->ring;
   birth_common(c, q, s->src, 1);
@@ -456,6 +469,11 @@ static void transport(ctx *c, part *q) {
     double dmx = plane_dist(p->mesh[0][q->mx], p->mesh[0][q->mx + 1], q->x, u0);
     double dmy = plane_dist(p->mesh[1][q->my], p->mesh[1][q->my + 1], q->y, v0);
     double dmz = plane_dist(p->mesh[2][q->mz], p->mesh[2][q->mz + 1], q->z, w0);
+    double vel = 0.0, dtm = INFINITY;                                   /* TD1, TD2: speed and distance to the next time edge */
+    if (p->n_t > 0) {
+      vel = p->G > 0 ? p->speed[q->g] : 1.3831592e6 * sqrt(q->E);
+      dtm = (p->t_edges[q->it + 1] - q->t) * vel;
+    }
     double ds = dx;
     if (dy < ds) ds = dy;
     if (dz < ds) ds = dz;
@@ -464,11 +482,13 @@ static void transport(ctx *c, part *q) {
     if (dmx < ds) ds = dmx;
     if (dmy < ds) ds = dmy;
     if (dmz < ds) ds = dmz;
+    if (dtm < ds) ds = dtm;
     int collide = dcoll < ds;                                           /* G5: surface wins ties */
     double d = collide ? dcoll : ds;
     if (!(d < INFINITY)) { c->err = ORC_ELOST; return; }
     /* T4 */
     q->x = q->x + d * u0; q->y = q->y + d * v0; q->z = q->z + d * w0;
+    if (p->n_t > 0) q->t = q->t + d / vel;                              /* TD3 */
     c->tot[ORC_T_NSEG] += 1;
     /* T5 */
     int e = -1;
@@ -479,13 +499,14 @@ static void transport(ctx *c, part *q) {
       e = lo;
     }
     size_t bin = 0;
-    if (e >= 0) bin = ((((size_t)q->mz * p->mesh_n[1] + q->my) * p->mesh_n[0]) + q->mx) * p->n_e + e;
-    if (c->active && e >= 0 && __builtin_add_overflow(c->flux[bin], fixp(p, d), &c->flux[bin])) { c->err = ORC_EOVERFLOW; return; }   /* N5 */
+    if (e >= 0) bin = (((((size_t)q->it * p->mesh_n[2] + q->mz) * p->mesh_n[1] + q->my) * p->mesh_n[0]) + q->mx) * p->n_e + e;   /* TD4: it = 0 without a time mesh */
+    const double wd = p->implicit ? q->wgt * d : d;                     /* W2: scores carry the weight (1 in analog runs) */
+    if (c->active && e >= 0 && __builtin_add_overflow(c->flux[bin], fixp(p, wd), &c->flux[bin])) { c->err = ORC_EOVERFLOW; return; }   /* N5 */
     if (c->kmode) c->P += fixp(p, d * nsf);
     if (collide) {
       /* T6 */
       q->ncoll += 1; c->tot[ORC_T_NCOLL] += 1;
-      if (c->active && e >= 0 && __builtin_add_overflow(c->coll[bin], fixp(p, 1.0), &c->coll[bin])) { c->err = ORC_EOVERFLOW; return; }
+      if (c->active && e >= 0 && __builtin_add_overflow(c->coll[bin], fixp(p, p->implicit ? q->wgt : 1.0), &c->coll[bin])) { c->err = ORC_EOVERFLOW; return; }
       if (c->kmode) c->Pc += fixp(p, nsf / St);
       int kind;                                                         /* 0 scatter 1 capture 2 fission */
       int fnuc = 0; double nu = 0.0; int src = mat;
@@ -493,6 +514,13 @@ static void transport(ctx *c, part *q) {
         double r = orc_draw(seed, q->id, gen, seg, PUR_SELECT, 1) * St;
         double sst = p->sst[mat * p->G + q->g];
         if (r < sst) kind = 0; else if (r < sst + p->sig_c[mat * p->G + q->g]) kind = 1; else kind = 2;
+        if (p->implicit) {                                               /* W3: capture by weight, then scatter or fission */
+          const double snc = St - p->sig_c[mat * p->G + q->g];
+          if (snc > 0.0) {
+            q->wgt = q->wgt * (snc / St);
+            kind = (orc_draw(seed, q->id, gen, seg, PUR_SELECT, 1) * snc < sst) ? 0 : 2;
+          } else kind = 1;
+        }
         nu = p->nu[mat * p->G + q->g];
       } else {
         double r = orc_draw(seed, q->id, gen, seg, PUR_SELECT, 0) * St;
@@ -501,6 +529,13 @@ static void transport(ctx *c, part *q) {
         fnuc = p->mat_nuc[mat * ORC_MAX_NUC + n];
         double r2 = orc_draw(seed, q->id, gen, seg, PUR_SELECT, 1) * st[n];
         if (r2 < ss[n]) kind = 0; else if (r2 < ss[n] + sc[n]) kind = 1; else kind = 2;
+        if (p->implicit) {                                               /* W3 */
+          const double snc = st[n] - sc[n];
+          if (snc > 0.0) {
+            q->wgt = q->wgt * (snc / st[n]);
+            kind = (orc_draw(seed, q->id, gen, seg, PUR_SELECT, 1) * snc < ss[n]) ? 0 : 2;
+          } else kind = 1;
+        }
         nu = p->nuc_nu[fnuc]; src = fnuc;
       }
       if (kind == 0) {
@@ -526,6 +561,16 @@ static void transport(ctx *c, part *q) {
           s.ix = (int16_t)q->ix; s.iy = (int16_t)q->iy; s.iz = (int16_t)q->iz;
           s.mx = (int16_t)q->mx; s.my = (int16_t)q->my; s.mz = (int16_t)q->mz;
           s.ring = (uint8_t)q->ring; s.src = (uint8_t)src; s.depth = (uint8_t)(c->kmode ? 0 : q->depth + 1);
+          s.it = (uint8_t)q->it;                                        /* TD5: secondaries inherit the time */
+          if (!c->kmode) {
+            if (c->stack.n >= c->stack_t_cap) {
+              size_t nc = c->stack_t_cap ? 2 * c->stack_t_cap : 1024;
+              double *nt = (double *)realloc(c->stack_t, nc * sizeof(double)), *nw = (double *)realloc(c->stack_w, nc * sizeof(double));
+              if (!nt || !nw) { c->err = ORC_ENOMEM; return; }
+              c->stack_t = nt; c->stack_w = nw; c->stack_t_cap = nc;
+            }
+            c->stack_t[c->stack.n] = q->t; c->stack_w[c->stack.n] = q->wgt;
+          }
           if (push_site(c->kmode ? &c->bank : &c->stack, &s)) { c->err = ORC_ENOMEM; return; }
         }
         c->tot[ORC_T_NSITES] += (uint64_t)n;
@@ -557,6 +602,15 @@ static void transport(ctx *c, part *q) {
       if (dmy == d) { if (v0 > 0.0) { q->y = p->mesh[1][q->my + 1]; if (q->my + 1 < p->mesh_n[1]) q->my += 1; } else { q->y = p->mesh[1][q->my]; if (q->my > 0) q->my -= 1; } }
       if (dmz == d) { if (w0 > 0.0) { q->z = p->mesh[2][q->mz + 1]; if (q->mz + 1 < p->mesh_n[2]) q->mz += 1; } else { q->z = p->mesh[2][q->mz]; if (q->mz > 0) q->mz -= 1; } }
       if (!alive) c->tot[ORC_T_NLEAK] += 1;
+      if (dtm == d) {                                                   /* TD3: time edge; the last one is the census */
+        q->t = p->t_edges[q->it + 1]; q->it += 1;
+        if (q->it == p->n_t && alive) { alive = 0; c->tot[ORC_T_NCENSUS] += 1; }
+      }
+    }
+    /* W4 closeout (the fifth event of the paper's decomposed scheme): weight roulette for the next segment */
+    if (p->implicit && alive && q->wgt < p->w_roulette) {
+      if (orc_draw(seed, q->id, gen, seg, PUR_CLOSEOUT, 0) * p->w_survive < q->wgt) q->wgt = p->w_survive;
+      else { alive = 0; c->tot[ORC_T_NROULETTE] += 1; }
     }
   }
   record_death(c, q);
@@ -583,11 +637,11 @@ static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, in
     for (uint64_t i = 0; i < n_src; i++) {
       if (c.err) continue;
       part q;
-      if (sites) birth_site(&c, &q, &sites[i]); else birth_primary(&c, &q, first_id + i);
+      if (sites) birth_site(&c, &q, &sites[i], 0.0, 1.0); else birth_primary(&c, &q, first_id + i);
       transport(&c, &q);
       while (!c.err && c.stack.n > 0) {                 /* D1: secondaries, LIFO, to extinction */
         orc_site s = c.stack.v[--c.stack.n];
-        birth_site(&c, &q, &s);
+        birth_site(&c, &q, &s, c.stack_t[c.stack.n], c.stack_w[c.stack.n]);
         transport(&c, &q);
       }
     }
@@ -615,7 +669,7 @@ static void run_batch(orc_problem *p, uint64_t seed, uint32_t gen, int kmode, in
         }
       }
     }
-    free(c.flux); free(c.coll); free(c.bank.v); free(c.stack.v); free(c.hist.id); free(c.hist.nseg); free(c.hist.ncoll);
+    free(c.flux); free(c.coll); free(c.bank.v); free(c.stack.v); free(c.stack_t); free(c.stack_w); free(c.hist.id); free(c.hist.nseg); free(c.hist.ncoll);
   }
 }
 
@@ -653,7 +707,7 @@ int orc_run_fixed_source(orc_problem *p, uint64_t n, uint64_t seed) { return orc
  * share of the source, runs its generation, the (P, Pc, N, M) sums are added over the processes, and every process
  * controls its own bank with the global p = N / M.  orc_run_k_eigenvalue is the same loop with one share. */
 int orc_k_begin(orc_problem *p, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed) {
-  if (!p || n_gen == 0 || n_gen > 65535) return ORC_EINVAL;
+  if (!p || n_gen == 0 || n_gen > 65535 || p->n_t > 0 || p->implicit) return ORC_EINVAL;      /* the time mesh belongs to fixed-source runs */
   int rc = alloc_results(p, n_gen); if (rc) return rc;
   free(p->ksrc); free(p->kbank); p->ksrc = NULL; p->kbank = NULL; p->n_kbank = 0;
   p->k_first = first_id; p->n_ksrc = n_local; p->kseed = seed;

@@ -57,6 +57,10 @@ typedef struct orc_geometry {
   int32_t src_index;                         /* group or nuclide */
   double src_energy;
   int32_t tally_scale_log2;
+  int32_t n_tbins;                           /* time-dependent fixed source: time bins (0 = time-independent) */
+  const double *t_edges;                     /* n_tbins+1 ascending; t_edges[0] = emission time, t_edges[n_tbins] = census */
+  int32_t implicit_capture;                  /* fixed source: capture by weight reduction + weight roulette (the closeout event) */
+  double w_roulette, w_survive;              /* roulette below w_roulette; survivors get w_survive */
 } orc_geometry;
 
 typedef struct orc_materials {
@@ -66,6 +70,7 @@ typedef struct orc_materials {
   const int32_t *mat_nnuc;                   /* CE: n_mat */
   const int32_t *mat_nuc;                    /* CE: n_mat*ORC_MAX_NUC */
   const double *mat_dens;                    /* CE: n_mat*ORC_MAX_NUC */
+  const double *speed;                       /* MG, time-dependent runs: speed of group g (cm per time unit), [G] */
 } orc_materials;
 
 typedef struct orc_xs_tables {
@@ -80,7 +85,7 @@ typedef struct orc_site {                    /* 48 bytes */
   double x, y, z;
   uint64_t id;
   int16_t ix, iy, iz, mx, my, mz;
-  uint8_t ring, src, depth, pad;
+  uint8_t ring, src, depth, it;             /* it: time bin (time-dependent fixed source), else 0 */
 } orc_site;
 
 typedef struct orc_sizes {
@@ -91,7 +96,7 @@ typedef struct orc_sizes {
 } orc_sizes;
 
 enum { ORC_T_NSEG = 0, ORC_T_NCOLL, ORC_T_NCROSS, ORC_T_NABS, ORC_T_NFIS, ORC_T_NLEAK,
-       ORC_T_NBORN, ORC_T_NDROPPED, ORC_T_NDIRFAIL, ORC_T_DIGEST, ORC_T_NSITES, ORC_T_COUNT = 12 };
+       ORC_T_NBORN, ORC_T_NDROPPED, ORC_T_NDIRFAIL, ORC_T_DIGEST, ORC_T_NSITES, ORC_T_NCENSUS, ORC_T_NROULETTE, ORC_T_COUNT = 16 };
 
 typedef struct orc_tallies {                 /* all buffers caller-allocated; NULL = skip */
   int64_t *flux, *coll;                      /* n_bins */

@@ -13,12 +13,12 @@ import numpy as np
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB = os.environ.get("ORC_LIB") or os.path.join(HERE, "liborc.so")     # ORC_LIB: tests/mutation_check.py loads a mutant
-MAX_RINGS, MAX_NUC, T_COUNT = 4, 4, 12
+MAX_RINGS, MAX_NUC, T_COUNT = 4, 4, 16
 TOTAL_NAMES = ["n_seg", "n_coll", "n_cross", "n_abs", "n_fis", "n_leak", "n_born", "n_dropped",
-               "n_dirfail", "digest", "n_sites"]
+               "n_dirfail", "digest", "n_sites", "n_census", "n_roulette"]
 SITE_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("id", "<u8"), ("ix", "<i2"), ("iy", "<i2"),
                        ("iz", "<i2"), ("mx", "<i2"), ("my", "<i2"), ("mz", "<i2"), ("ring", "u1"),
-                       ("src", "u1"), ("depth", "u1"), ("pad", "u1")])
+                       ("src", "u1"), ("depth", "u1"), ("it", "u1")])
 assert SITE_DTYPE.itemsize == 48
 
 PD, PI = C.POINTER(C.c_double), C.POINTER(C.c_int32)
@@ -43,12 +43,13 @@ class Geometry(C.Structure):
                 ("src_kind", C.c_int32), ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3),
                 ("src_dir_kind", C.c_int32), ("src_dir", C.c_double * 3),
                 ("src_energy_kind", C.c_int32), ("src_index", C.c_int32), ("src_energy", C.c_double),
-                ("tally_scale_log2", C.c_int32)]
+                ("tally_scale_log2", C.c_int32), ("n_tbins", C.c_int32), ("t_edges", PD),
+                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double)]
 
 
 class Materials(C.Structure):
     _fields_ = [("n_mat", C.c_int32), ("G", C.c_int32), ("sig_t", PD), ("sig_s", PD), ("sig_f", PD), ("nu", PD),
-                ("chi", PD), ("mat_nnuc", PI), ("mat_nuc", PI), ("mat_dens", PD)]
+                ("chi", PD), ("mat_nnuc", PI), ("mat_nuc", PI), ("mat_dens", PD), ("speed", PD)]
 
 
 class XsTables(C.Structure):

@@ -12,6 +12,7 @@
 #include "tdr_async.cuh"
 #include "tdr_pstash.cuh"
 #include "tdr_cstash.cuh"
+#include "tdr_peaks.cuh"
 
 static thread_local char g_err[512] = "";
 static int fail(int code, const char *fmt, ...) {
@@ -50,7 +51,7 @@ struct tdr_problem {
   // workspace
   char *ws = nullptr; u64 ws_bytes = 0; cudaStream_t stream = nullptr;
   // carved pointers (valid during/after a run)
-  Soa soa; u32 *stacks[EV_COUNT]; u64 *ctr; DevOut out; tdr_site *bank, *srcbank, *sec;
+  Soa soa; u32 *stacks[EV_COUNT]; u64 *ctr; DevOut out; tdr_site *bank, *srcbank, *sec; double *sec_time = nullptr, *sec_w = nullptr;
   u64 bank_cap = 0, src_cap = 0, sec_cap = 0, hist_cap = 0, W = 0;
   u64 *hist_id; u32 *hist_nseg, *hist_ncoll;
   AsyncMem am; PsMem pm;
@@ -94,6 +95,14 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
   if (m->n_mat > 255 || m->G > 255 || m->G < 0) return fail(TDR_EINVAL, "too many materials or groups");
   if (m->G == 0 && !x) return fail(TDR_EINVAL, "continuous energy needs xs_tables");
   if (g->tally_scale_log2 < 0 || g->tally_scale_log2 > 40) return fail(TDR_EINVAL, "tally_scale_log2 out of range");
+  if (g->n_tbins < 0 || g->n_tbins > 255) return fail(TDR_EINVAL, "n_tbins in [0,255]");
+  if (g->implicit_capture && !(g->w_roulette > 0.0 && g->w_survive >= g->w_roulette)) return fail(TDR_EINVAL, "implicit capture needs 0 < w_roulette <= w_survive");
+  if (g->n_tbins > 0) {
+    if (!g->t_edges) return fail(TDR_EINVAL, "time mesh without t_edges");
+    for (int k = 0; k < g->n_tbins; k++) if (!(g->t_edges[k] < g->t_edges[k + 1])) return fail(TDR_EINVAL, "time edges are not strictly ascending");
+    if (m->G > 0 && !m->speed) return fail(TDR_EINVAL, "a multigroup time-dependent run needs group speeds");
+    if (m->G > 0) for (int a = 0; a < m->G; a++) if (!(m->speed[a] > 0.0)) return fail(TDR_EINVAL, "group speeds must be positive");
+  }
   const double *mp[3] = { g->mesh_x, g->mesh_y, g->mesh_z };
   const double *lp[3] = { g->xplanes, g->yplanes, g->zplanes };
   const int ln[3] = { g->nx, g->ny, g->nz };
@@ -168,6 +177,8 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
   UP(g->univ_nrings, g->n_univ, D.univ_nr); UP(g->univ_radius, g->n_univ * TDR_MAX_RINGS, D.univ_rad);
   UP(g->univ_mat, g->n_univ * (TDR_MAX_RINGS + 1), D.univ_mat);
   for (int a = 0; a < 3; a++) UP(mp[a], g->mesh_n[a] + 1, D.mesh[a]);
+  D.n_t = g->n_tbins; D.implicit = g->implicit_capture != 0; D.w_roulette = g->w_roulette; D.w_survive = g->w_survive;
+  if (D.n_t > 0) { UP(g->t_edges, D.n_t + 1, D.t_edges); if (m->G > 0) UP(m->speed, m->G, D.speed); }
   D.src_kind = g->src_kind; D.src_dir_kind = g->src_dir_kind; D.src_energy_kind = g->src_energy_kind; D.src_index = g->src_index;
   memcpy(D.src_lo, g->src_lo, 24); memcpy(D.src_hi, g->src_hi, 24); memcpy(D.src_dir, g->src_dir, 24);
   D.src_energy = g->src_energy; D.scale = ldexp(1.0, g->tally_scale_log2); p->S = g->tally_scale_log2;
@@ -216,7 +227,7 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
   }
 #undef UP
   if (rc) { tdr_free_problem(p); return rc; }
-  D.n_bins = (u64)D.mesh_n[0] * D.mesh_n[1] * D.mesh_n[2] * D.n_e;
+  D.n_bins = (u64)(D.n_t > 0 ? D.n_t : 1) * D.mesh_n[0] * D.mesh_n[1] * D.mesh_n[2] * D.n_e;
   cudaDeviceProp prop; int dev = 0; cudaGetDevice(&dev);
   if (cudaGetDeviceProperties(&prop, dev) == cudaSuccess) p->num_sms = prop.multiProcessorCount;
   if (cudaMallocHost((void **)&p->h_ctr, 64 * sizeof(u64)) != cudaSuccess) { tdr_free_problem(p); return fail(TDR_ECUDA, "cudaMallocHost failed"); }
@@ -272,6 +283,8 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   s.x = c.take<double>(W); s.y = c.take<double>(W); s.z = c.take<double>(W);
   s.u = c.take<double>(W); s.v = c.take<double>(W); s.w = c.take<double>(W);
   s.E = c.take<double>(p->ce ? W : 1);
+  s.t = p->dp.n_t > 0 ? c.take<double>(W) : nullptr;
+  s.wgt = p->dp.implicit ? c.take<double>(W) : nullptr;
   s.id = c.take<u64>(W); s.loc0 = c.take<u64>(W); s.loc1 = c.take<u64>(W);
   s.seg = c.take<u32>(W); s.ncoll = c.take<u32>(W);
   s.s_sigt = c.take<double>(W); s.s_nsf = c.take<double>(W); s.s_d = c.take<double>(W); s.s_f = c.take<double>(W);
@@ -284,13 +297,14 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   o.totals = c.take<u64>(TDR_T_COUNT); o.PPc = c.take<u64>(2); o.err = c.take<int>(1);
   u64 bank_cap = p->bank_cap_opt ? p->bank_cap_opt : 2 * n + n / 2 + 4096, src_cap = n + n / 4 + 4096, sec_cap = W + (1ull << 20);
   tdr_site *bank = c.take<tdr_site>(bank_cap), *src = c.take<tdr_site>(src_cap), *sec = c.take<tdr_site>(sec_cap);
+  double *sec_time = p->dp.n_t > 0 ? c.take<double>(sec_cap) : nullptr, *sec_w = p->dp.implicit ? c.take<double>(sec_cap) : nullptr;
   u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
   u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
   AsyncMem am; async_layout(c, W, sec_cap, p->arena_links_opt, am);
   PsMem pm; pstash_layout(c, W, p->arena_links_opt, pm);
   if (assign) {
     p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
-    p->bank = bank; p->srcbank = src; p->sec = sec; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
+    p->bank = bank; p->srcbank = src; p->sec = sec; p->sec_time = sec_time; p->sec_w = sec_w; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
     p->hist_cap = hist_cap; p->hist_id = hid; p->hist_nseg = hs; p->hist_ncoll = hc; p->am = am; p->pm = pm;
   }
   return (c.off + 255) & ~255ull;
@@ -337,7 +351,8 @@ static void collect_kernel_times(tdr_problem *p) {
 
 static int check_dev_err(tdr_problem *p, int code) {
   if (code == 0) return 0;
-  const char *w = code == TDR_ECAPACITY ? "bank/stack/arena capacity exceeded" : code == TDR_ELOST ? "lost particle (no finite distance or segment overflow)" : "device error";
+  const char *w = code == TDR_ECAPACITY ? "bank/stack/arena capacity exceeded" : code == TDR_ELOST ? "lost particle (no finite distance or segment overflow)" :
+                  code == TDR_EOVERFLOW ? "a fixed-point tally left int64 (lower tally_scale_log2)" : "device error";
   return fail(code, "%s", w);
 }
 
@@ -438,12 +453,14 @@ static int run_stack(tdr_problem *p, DevRun R) {
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
     h_sec_head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;          // claims past the limit got nothing
     const u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
-    if (!split && R.kmode && rem == 0 && alive > 0 && alive <= (u64)p->drain_below) {
-      // tail drain: the few particles left are followed to their death in ONE launch (k_drain)
+    if (R.kmode && rem == 0 && alive > 0 && alive <= (u64)p->drain_below) {
+      // tail drain: the few particles left are followed to their death in ONE launch (k_drain).  Also under the five-event
+      // decomposition: after a whole iteration every survivor waits on the LOOKUP stack, i.e. at the start of a segment.
       const int blocks = (int)((alive + 63) / 64);
       {
         KTimer td(p, true);
-        k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + it % 3);
+        if (split) k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP);
+        else k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + it % 3);
       }
       LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.iterations++;
       CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
@@ -579,6 +596,9 @@ static int run_cstash(tdr_problem *p, DevRun R) {
   return 0;
 }
 
+static int overflow_check(tdr_problem *p);
+static int run_async_any(tdr_problem *p, DevRun &R);
+
 // one generation (or the whole fixed-source run) under the selected scheme
 static int run_generation(tdr_problem *p, DevRun &R) {
   cudaStream_t st = p->stream;
@@ -586,13 +606,26 @@ static int run_generation(tdr_problem *p, DevRun &R) {
   CK(cudaMemsetAsync(p->out.PPc, 0, 16, st));
   R.src_next = p->ctr + C_SRC_NEXT; R.sec_tail = p->ctr + C_SEC_TAIL; R.sec_head = p->ctr + C_SEC_HEAD;
   R.bank_count = p->ctr + C_BANK; R.hist_count = p->ctr + C_HIST;
-  R.sec = p->sec; R.sec_cap = p->sec_cap; R.sec_limit = 0; R.sec_head0 = 0;
+  R.sec = p->sec; R.sec_time = p->sec_time; R.sec_w = p->sec_w; R.sec_cap = p->sec_cap; R.sec_limit = 0; R.sec_head0 = 0;
   R.bank = p->bank; R.bank_cap = p->bank_cap;
   R.hist_id = p->hist_id; R.hist_nseg = p->hist_nseg; R.hist_ncoll = p->hist_ncoll;
-  if (p->scheme == 0) return p->ce ? run_stack<true>(p, R) : run_stack<false>(p, R);
+  if (p->scheme == 0) { int rc = p->ce ? run_stack<true>(p, R) : run_stack<false>(p, R); return rc ? rc : overflow_check(p); }
+  { int rc = run_async_any(p, R); return rc ? rc : overflow_check(p); }
+}
+
+static int overflow_check(tdr_problem *p) {
+  if (p->dp.n_bins <= PRIV_MAX_BINS) return 0;               // block-private tallies are checked at every flush; the scheme's own read-back saw the flag
+  k_overflow_check<<<64, 256, 0, p->stream>>>(p->out.flux, p->out.coll, p->dp.n_bins, p->out.err);
+  LAUNCH_CHECK();
+  CK(cudaMemcpyAsync(p->h_ctr + 32, p->out.err, sizeof(int), cudaMemcpyDeviceToHost, p->stream)); CK(cudaStreamSynchronize(p->stream));
+  return check_dev_err(p, *(int *)(p->h_ctr + 32));
+}
+
+static int run_async_any(tdr_problem *p, DevRun &R) {
   // auto: the shared particle stash where the path is instruction bound (multigroup); the index stash where it is bound by
   // cross-section gathers and wants the L1 that a particle stash would take (continuous energy) — DESIGN.md section 6
-  const int stash = p->stash >= 0 ? p->stash : (p->ce ? 0 : 2);
+  if ((p->dp.n_t > 0 || p->dp.implicit) && p->stash > 0) return fail(TDR_EINVAL, "time-dependent and implicit-capture runs use the index stash (stash = auto|index)");
+  const int stash = p->stash >= 0 ? p->stash : ((p->ce || p->dp.n_t > 0 || p->dp.implicit) ? 0 : 2);
   if (stash == 2 && p->split != 1) return p->ce ? run_cstash<true>(p, R) : run_cstash<false>(p, R);
   if (stash == 1 && p->split != 1) return p->ce ? run_pstash<true>(p, R) : run_pstash<false>(p, R);
   return p->ce ? run_async<true>(p, R) : run_async<false>(p, R);      // index stash; the five-event decomposition always
@@ -642,6 +675,7 @@ int tdr_run_fixed_source(tdr_problem *p, uint64_t n, uint64_t seed) {
 // ---------------------------------------------------------------------------------- D2 in steps (one problem on several GPUs)
 int tdr_k_begin(tdr_problem *p, uint64_t first_id, uint64_t n_local, uint32_t n_gen, uint64_t seed) {
   if (n_gen == 0 || n_gen > 65535) return fail(TDR_EINVAL, "bad generation counts");
+  if (p && (p->dp.n_t > 0 || p->dp.implicit)) return fail(TDR_EINVAL, "the time mesh and implicit capture belong to fixed-source runs");
   int rc = begin_run(p, n_local ? n_local : 1); if (rc) return rc;
   p->k_first = first_id; p->k_nsrc = n_local; p->k_seed = seed; p->k_ngen = n_gen; p->k_last_bank = 0;
   p->k_keep = p->keep_history < 0 ? n_local <= 2000000 : p->keep_history != 0;
@@ -775,5 +809,43 @@ int tdr_dev_det_log(const double *x, double *out, uint64_t n, void *stream) {
 int tdr_dev_draw(uint64_t seed, const uint64_t *id, uint32_t gen, uint32_t seg, uint32_t purpose, uint32_t j, double *out, uint64_t n, void *stream) {
   k_draw<<<296, 256, 0, (cudaStream_t)stream>>>(seed, (const u64 *)id, gen, seg, purpose, j, out, n);
   CK(cudaGetLastError()); CK(cudaStreamSynchronize((cudaStream_t)stream));
+  return TDR_OK;
+}
+
+// what: 0 = fp64 DFMA rate in TFLOP/s, 1 = L2-resident copy bandwidth in GB/s (read + write).  Uses its own scratch memory.
+int tdr_measure_peak(int what, double *value, void *stream) {
+  if (!value || what < 0 || what > 1) return fail(TDR_EINVAL, "bad argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaDeviceProp prop; int dev = 0; CK(cudaGetDevice(&dev)); CK(cudaGetDeviceProperties(&prop, dev));
+  const int sms = prop.multiProcessorCount;
+  cudaEvent_t e0, e1; CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+  float best = 1e30f; double work = 0.0;
+  if (what == 0) {
+    const int grid = sms * 8, iters = 1 << 16;
+    double *out = nullptr; CK(cudaMalloc(&out, (size_t)grid * 256 * 8));
+    for (int r = 0; r < 4; r++) {
+      CK(cudaEventRecord(e0, st));
+      k_peak_dfma<<<grid, 256, 0, st>>>(out, iters, 1.0000001, 1e-9);
+      CK(cudaEventRecord(e1, st)); CK(cudaEventSynchronize(e1));
+      float ms = 0; CK(cudaEventElapsedTime(&ms, e0, e1)); if (r > 0 && ms < best) best = ms;
+    }
+    CK(cudaFree(out));
+    work = 2.0 * 8.0 * iters * (double)grid * 256.0 / 1e12;                 // TFLOP
+  } else {
+    const size_t n = (size_t)1 << 20;                                        // 16 MB in + 16 MB out
+    const int reps = 64;
+    double2 *buf = nullptr; CK(cudaMalloc(&buf, 2 * n * sizeof(double2))); CK(cudaMemsetAsync(buf, 0, 2 * n * sizeof(double2), st));
+    for (int r = 0; r < 4; r++) {
+      CK(cudaEventRecord(e0, st));
+      k_peak_copy<<<sms * 8, 256, 0, st>>>(buf, buf + n, n, reps);
+      CK(cudaEventRecord(e1, st)); CK(cudaEventSynchronize(e1));
+      float ms = 0; CK(cudaEventElapsedTime(&ms, e0, e1)); if (r > 0 && ms < best) best = ms;
+    }
+    CK(cudaFree(buf));
+    work = 2.0 * (double)n * sizeof(double2) * reps / 1e9;                   // GB
+  }
+  CK(cudaGetLastError());
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *value = work / (best / 1e3);
   return TDR_OK;
 }

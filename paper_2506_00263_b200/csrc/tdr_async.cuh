@@ -229,7 +229,7 @@ __device__ __forceinline__ bool make_work_async(const DevProb &P, const double *
       const u64 idx = h + rank, k = idx % R.sec_cap;
       bool ok = true;                                              // its writer is between the ticket and the flag
       while (ld_vol(&A.sec_flag[k]) != idx + 1) { if (*(volatile int *)err) { ok = false; break; } __nanosleep(20); }
-      if (ok) { __threadfence(); tdr_site s = R.sec[k]; birth_site<CE>(P, mg, R, acc, p, s); reborn = true; }
+      if (ok) { __threadfence(); tdr_site s = R.sec[k]; birth_site<CE>(P, mg, R, acc, p, s, R.sec_time ? R.sec_time[k] : 0.0, R.sec_w ? R.sec_w[k] : 1.0); reborn = true; }
     }
     m = __ballot_sync(FULL, want && !reborn);
     if (m == 0) return reborn;

@@ -71,6 +71,20 @@ struct CsPool {                             // NS slots, SoA; then three rings o
     base = __shfl_sync(FULL, base, leader);
     if (pred) ring[r][(base + __popc(m & lanemask_lt())) & mask] = (unsigned short)slot;
   }
+  // every lane's slot goes to at most one of the three rings: lanes 0, 1, 2 reserve the three ranges with ONE atomic
+  // instruction (three addresses), instead of three dependent ballot / atomic / shuffle rounds
+  __device__ __forceinline__ void push3(CsCtl *c, u32 slot, bool to_move, bool to_collide, bool to_birth) const {
+    const u32 mM = __ballot_sync(FULL, to_move), mC = __ballot_sync(FULL, to_collide), mB = __ballot_sync(FULL, to_birth);
+    const u32 lane = threadIdx.x & 31;
+    const u32 cnt = (u32)__popc(lane == 0 ? mM : lane == 1 ? mC : mB);
+    u32 base = 0;
+    if (lane < 3 && cnt) base = atomicAdd(&c->tail[lane], cnt);
+    const u32 bM = __shfl_sync(FULL, base, 0), bC = __shfl_sync(FULL, base, 1), bB = __shfl_sync(FULL, base, 2);
+    const u32 lt = lanemask_lt();
+    if (to_move) ring[CE_MOVE][(bM + __popc(mM & lt)) & mask] = (unsigned short)slot;
+    else if (to_collide) ring[CE_COLLIDE][(bC + __popc(mC & lt)) & mask] = (unsigned short)slot;
+    else if (to_birth) ring[CE_BIRTH][(bB + __popc(mB & lt)) & mask] = (unsigned short)slot;
+  }
 };
 
 // k-mode fission sites -> bank, one child per lane (the batch's children are spread over the warp, so the id derivation
@@ -237,8 +251,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
         }
       }
       if (born) pl.store(slot, p);
-      pl.push(&ctl, CE_MOVE, slot, born);
-      pl.push(&ctl, CE_BIRTH, slot, valid && !born);
+      pl.push3(&ctl, slot, born, false, valid && !born);
       if (!R.kmode && w.open_count != open_pub) { if (lane == 0) atomicAdd(&ctl.open_total, w.open_count - open_pub); open_pub = w.open_count; }
       ev_cnt[CE_BIRTH]++; ln_cnt[CE_BIRTH] += __popc(__ballot_sync(FULL, born));
       continue;
@@ -268,9 +281,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
         if (ncw) { if (R.kmode) cs_push_children_bank(O, R, &acc, p, nch, csrc); else { ps_push_secondaries(w, R, &acc, p, nch, csrc); delta += (i64)ncw; } }
       }
       delta -= (i64)__popc(__ballot_sync(FULL, died));
-      pl.push(&ctl, CE_MOVE, slot, alive);
-      if (MODE == 2) pl.push(&ctl, CE_COLLIDE, slot, tocoll);
-      pl.push(&ctl, CE_BIRTH, slot, valid && !alive && !tocoll);
+      pl.push3(&ctl, slot, alive, tocoll, valid && !alive && !tocoll);
       ev_cnt[CE_MOVE]++; ln_cnt[CE_MOVE] += n;
     } else {
       // ------------------------------------------------------------------ COLLIDE: T6 on a full warp of colliders
@@ -290,8 +301,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
       if (ncw) { if (R.kmode) cs_push_children_bank(O, R, &acc, p, nch, csrc); else { ps_push_secondaries(w, R, &acc, p, nch, csrc); delta += (i64)ncw; } }
       const bool died = valid && !alive;
       delta -= (i64)__popc(__ballot_sync(FULL, died));
-      pl.push(&ctl, CE_MOVE, slot, alive);
-      pl.push(&ctl, CE_BIRTH, slot, died);
+      pl.push3(&ctl, slot, alive, false, died);
       ev_cnt[CE_COLLIDE]++; ln_cnt[CE_COLLIDE] += n;
     }
     if (!R.kmode) {

@@ -10,7 +10,7 @@
 #define FULL 0xFFFFFFFFu
 
 enum { PUR_DIST = 0, PUR_SELECT = 1, PUR_ENERGY = 2, PUR_DIR = 3, PUR_MULT = 4, PUR_POS = 5, PUR_POPCTRL = 6,
-       PUR_IDDERIVE = 15 };
+       PUR_CLOSEOUT = 7, PUR_IDDERIVE = 15 };
 #define MAX_ATTEMPT 1024
 
 typedef unsigned long long u64;
@@ -19,12 +19,13 @@ typedef unsigned int u32;
 
 // ---------------------------------------------------------------------------------- problem on the device
 struct DevProb {
-  int nx, ny, nz, n_univ, G, n_mat, n_e, by_group, n_grid, n_nuc;
+  int nx, ny, nz, n_univ, G, n_mat, n_e, by_group, n_grid, n_nuc, n_t;      // n_t: time bins (0 = time-independent)
   int bc[6], mesh_n[3];
-  const double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges;
+  const double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges, *t_edges, *speed;
   const int *cell_univ, *univ_nr, *univ_mat;
   int src_kind, src_dir_kind, src_energy_kind, src_index;
   double src_lo[3], src_hi[3], src_dir[3], src_energy, scale;
+  int implicit; double w_roulette, w_survive;   // W: implicit capture + weight roulette (fixed source)
   // MG table (staged to shared memory): per (m,g) row of MGROW doubles, then chi cdf per material
   const double *mg; int mg_doubles;
   // CE
@@ -44,7 +45,7 @@ struct DevOut {
 };
 
 struct Soa {                                  // particle state, one array per field
-  double *x, *y, *z, *u, *v, *w, *E;
+  double *x, *y, *z, *u, *v, *w, *E, *t, *wgt; // t: time-dependent runs only, wgt: implicit capture only (else nullptr)
   u64 *id, *loc0, *loc1;
   u32 *seg, *ncoll;
   double *s_sigt, *s_nsf, *s_d, *s_f;        // split-decomposition scratch
@@ -54,7 +55,7 @@ struct Soa {                                  // particle state, one array per f
 struct DevRun {
   u64 seed; u32 gen; int kmode, active; double k_prev;
   int src_sites; const tdr_site *sites; u64 src_total; u64 *src_next;
-  tdr_site *sec; u64 sec_cap; u64 *sec_tail, *sec_head; u64 sec_limit, sec_head0;   // fixed-source secondaries (ring):
+  tdr_site *sec; double *sec_time, *sec_w; u64 sec_cap; u64 *sec_tail, *sec_head; u64 sec_limit, sec_head0;   // fixed-source secondaries (ring):
                                                   // records [sec_head0, sec_limit) are complete and claimable
   tdr_site *bank; u64 bank_cap; u64 *bank_count;                        // k-mode fission bank
   u64 *hist_id; u32 *hist_nseg, *hist_ncoll; u64 *hist_count; u64 hist_cap;
@@ -66,9 +67,9 @@ struct DevRun {
 };
 
 struct Part {
-  double x, y, z, u, v, w, E;
+  double x, y, z, u, v, w, E, t, wgt;
   u64 id;
-  int ix, iy, iz, ring, depth, mx, my, mz, g;
+  int ix, iy, iz, ring, depth, mx, my, mz, g, it;
   u32 seg, ncoll;
 };
 
@@ -259,20 +260,20 @@ __device__ __forceinline__ void unpack_loc(Part &p, u64 l0, u64 l1) {
   p.ix = (int)(short)(l0 & 0xFFFF); p.iy = (int)(short)((l0 >> 16) & 0xFFFF); p.iz = (int)(short)((l0 >> 32) & 0xFFFF);
   p.ring = (int)((l0 >> 48) & 0xFF); p.depth = (int)((l0 >> 56) & 0xFF);
   p.mx = (int)(short)(l1 & 0xFFFF); p.my = (int)(short)((l1 >> 16) & 0xFFFF); p.mz = (int)(short)((l1 >> 32) & 0xFFFF);
-  p.g = (int)((l1 >> 48) & 0xFF);
+  p.g = (int)((l1 >> 48) & 0xFF); p.it = (int)((l1 >> 56) & 0xFF);
 }
 __device__ __forceinline__ u64 pack_loc0(const Part &p) {
   return (u64)(p.ix & 0xFFFF) | ((u64)(p.iy & 0xFFFF) << 16) | ((u64)(p.iz & 0xFFFF) << 32) |
          ((u64)(p.ring & 0xFF) << 48) | ((u64)(p.depth & 0xFF) << 56);
 }
 __device__ __forceinline__ u64 pack_loc1(const Part &p) {
-  return (u64)(p.mx & 0xFFFF) | ((u64)(p.my & 0xFFFF) << 16) | ((u64)(p.mz & 0xFFFF) << 32) | ((u64)(p.g & 0xFF) << 48);
+  return (u64)(p.mx & 0xFFFF) | ((u64)(p.my & 0xFFFF) << 16) | ((u64)(p.mz & 0xFFFF) << 32) | ((u64)(p.g & 0xFF) << 48) | ((u64)(p.it & 0xFF) << 56);
 }
 
 template <bool CE>
 __device__ __forceinline__ void load_part(const Soa &s, u32 i, Part &p) {
   p.x = s.x[i]; p.y = s.y[i]; p.z = s.z[i]; p.u = s.u[i]; p.v = s.v[i]; p.w = s.w[i];
-  p.E = CE ? s.E[i] : 0.0;
+  p.E = CE ? s.E[i] : 0.0; p.t = s.t ? s.t[i] : 0.0; p.wgt = s.wgt ? s.wgt[i] : 1.0;
   p.id = s.id[i]; p.seg = s.seg[i]; p.ncoll = s.ncoll[i];
   unpack_loc(p, s.loc0[i], s.loc1[i]);
 }
@@ -280,6 +281,8 @@ template <bool CE>
 __device__ __forceinline__ void store_part(const Soa &s, u32 i, const Part &p) {
   s.x[i] = p.x; s.y[i] = p.y; s.z[i] = p.z; s.u[i] = p.u; s.v[i] = p.v; s.w[i] = p.w;
   if (CE) s.E[i] = p.E;
+  if (s.t) s.t[i] = p.t;
+  if (s.wgt) s.wgt[i] = p.wgt;
   s.id[i] = p.id; s.seg[i] = p.seg; s.ncoll[i] = p.ncoll;
   s.loc0[i] = pack_loc0(p); s.loc1[i] = pack_loc1(p);
 }

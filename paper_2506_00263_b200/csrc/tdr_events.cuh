@@ -5,7 +5,7 @@
 #include "tdr_device.cuh"
 
 // flags produced by MOVE
-enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512 };
+enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512, F_TIME = 1024 };
 
 // per-block accumulators in shared memory, flushed once per kernel (finalize hook).  Every 64-bit sum
 // is two 32-bit words updated with native shared atomics: the carry out of the low word goes to the high word, so
@@ -45,7 +45,10 @@ __device__ __forceinline__ void acc_flush(BlockAcc *a, const DevOut &o, i64 P, i
   int t = threadIdx.x;
   if (t < TDR_T_COUNT + 2) {
     u64 v = ((u64)a->hi[t] << 32) + a->lo[t];
-    if (v) atomicAdd(t < TDR_T_COUNT ? &o.totals[t] : &o.PPc[t - TDR_T_COUNT], v);
+    if (v) {
+      const u64 old = atomicAdd(t < TDR_T_COUNT ? &o.totals[t] : &o.PPc[t - TDR_T_COUNT], v);
+      if (t >= TDR_T_COUNT && ((old + v) >> 63 || old + v < old)) atomicExch(o.err, TDR_EOVERFLOW);   // N5: P, Pc left int64
+    }
   } else if (t < TDR_T_COUNT + 8) { if (a->leak[t - TDR_T_COUNT - 2]) atomicAdd(&o.leak[t - TDR_T_COUNT - 2], (u64)a->leak[t - TDR_T_COUNT - 2]); }
 }
 
@@ -66,8 +69,9 @@ __device__ __forceinline__ void priv_add(u32 *lo, u32 *hi, u32 bin, u64 val) { a
 __device__ __forceinline__ void priv_flush(const TallyPriv &t, const DevOut &o) {   // after __syncthreads()
   for (int i = threadIdx.x; i < t.n; i += blockDim.x) {
     u64 f = ((u64)t.flux_hi[i] << 32) | t.flux_lo[i], c = ((u64)t.coll_hi[i] << 32) | t.coll_lo[i];
-    if (f) atomicAdd(&o.flux[i], f);
-    if (c) atomicAdd(&o.coll[i], c);
+    // N5: scores are non-negative, so a fixed-point sum that reaches 2^63 (or wraps) has left int64: an error, not a wrap
+    if (f) { const u64 old = atomicAdd(&o.flux[i], f); if ((old + f) >> 63 || old + f < old) atomicExch(o.err, TDR_EOVERFLOW); }
+    if (c) { const u64 old = atomicAdd(&o.coll[i], c); if ((old + c) >> 63 || old + c < old) atomicExch(o.err, TDR_EOVERFLOW); }
   }
 }
 
@@ -157,6 +161,11 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   double dmx = (mxl == xl && mxh == xh) ? dx : plane_dist(mxl, mxh, p.x, p.u);
   double dmy = (myl == yl && myh == yh) ? dy : plane_dist(myl, myh, p.y, p.v);
   double dmz = (mzl == zl && mzh == zh) ? dz : plane_dist(mzl, mzh, p.z, p.w);
+  double vel = 0.0, dtm = TDR_INF;                                    // TD1, TD2: speed, distance to the next time edge
+  if (P.n_t > 0) {
+    vel = P.G > 0 ? P.speed[p.g] : 1.3831592e6 * sqrt(p.E);
+    dtm = (P.t_edges[p.it + 1] - p.t) * vel;
+  }
   double ds = dx;
   if (dy < ds) ds = dy;
   if (dz < ds) ds = dz;
@@ -165,14 +174,16 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   if (dmx < ds) ds = dmx;
   if (dmy < ds) ds = dmy;
   if (dmz < ds) ds = dmz;
+  if (dtm < ds) ds = dtm;
   bool collide = dcoll < ds;                                           // G5
   d = collide ? dcoll : ds;
   flags = 0;
   if (!(d < TDR_INF)) { flags = F_LOST; d = 0.0; return; }
   if (collide) flags = F_COLLIDE;
   else flags = (dx == d ? F_DX : 0) | (dy == d ? F_DY : 0) | (dz == d ? F_DZ : 0) | (dout == d ? F_DOUT : 0) |
-               (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0);
+               (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0) | (dtm == d ? F_TIME : 0);
   p.x = p.x + d * p.u; p.y = p.y + d * p.v; p.z = p.z + d * p.w;       // G6
+  if (P.n_t > 0) p.t = p.t + d / vel;                                  // TD3
 }
 
 // ---------------------------------------------------------------------------------- T5 TALLY (warp-cooperative)
@@ -193,9 +204,10 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
   if (R.kmode && valid) { accP += fixp(d * nsf, P.scale); if (collide && nsf != 0.0) accPc += fixp(nsf / St, P.scale); }
   if (R.active) {
     u64 bin = 0;
-    if (e >= 0) bin = ((((u64)p.mz * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;
-    tally_add(o.flux, tp.flux_lo, tp.flux_hi, tp.n > 0, bin, fixp(d, P.scale), e >= 0);
-    tally_add(o.coll, tp.coll_lo, tp.coll_hi, tp.n > 0, bin, fixp(1.0, P.scale), e >= 0 && collide);
+    if (e >= 0) bin = (((((u64)p.it * P.mesh_n[2] + p.mz) * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;     // TD4
+    // W2: scores carry the weight (identically 1 in analog runs)
+    tally_add(o.flux, tp.flux_lo, tp.flux_hi, tp.n > 0, bin, fixp(P.implicit ? p.wgt * d : d, P.scale), e >= 0);
+    tally_add(o.coll, tp.coll_lo, tp.coll_hi, tp.n > 0, bin, fixp(P.implicit ? p.wgt : 1.0, P.scale), e >= 0 && collide);
   }
 }
 
@@ -236,6 +248,17 @@ __device__ TDR_COLD void record_deaths_warp(BlockAcc *a, const DevRun &R, bool v
   }
 }
 
+// ---------------------------------------------------------------------------------- W4 CLOSEOUT
+// "handles weights and weight windows for the particle's next loop iteration": weight roulette below w_roulette.  It runs
+// at the tail of the COLLIDE and SURFACE events (the two that end a segment) under every decomposition; analog runs
+// (weights identically 1) skip it on a uniform branch.
+__device__ __forceinline__ bool ev_closeout(const DevProb &P, const DevRun &R, BlockAcc *acc, Part &p) {
+  if (!P.implicit || !(p.wgt < P.w_roulette)) return true;
+  if (draw(R.seed, p.id, R.gen, p.seg, PUR_CLOSEOUT, 0) * P.w_survive < p.wgt) { p.wgt = P.w_survive; return true; }
+  record_death(acc, R, p, TDR_T_NROULETTE);
+  return false;
+}
+
 // ---------------------------------------------------------------------------------- T6 COLLIDE
 // returns true if the particle survives; n_children / child_src set on fission
 template <bool CE>
@@ -250,11 +273,16 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
     const double *row = mg + (mat * P.G + p.g) * MGROW(P.G);
     double r = draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * St;
     if (r < row[1]) kind = 0; else if (r < row[1] + row[2]) kind = 1; else kind = 2;
+    if (P.implicit) {                                                  // W3: capture by weight, then scatter or fission
+      const double snc = St - row[2];
+      if (snc > 0.0) { p.wgt = p.wgt * (snc / St); kind = (draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * snc < row[1]) ? 0 : 2; }
+      else kind = 1;
+    }
     nu = row[4]; child_src = mat;
     if (kind == 0) {
       p.g = sample_cdf(row + 5, P.G, draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0));
       if (iso_dir(seed, p.id, gen, p.seg, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
-      return true;
+      return ev_closeout(P, R, acc, p);
     }
   } else {
     Blk sb = rng_block(seed, p.id, gen, p.seg, PUR_SELECT, 0);
@@ -271,8 +299,13 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
     }
     double r2 = blk_odd(sb) * st;
     if (r2 < ss) kind = 0; else if (r2 < ss + sc) kind = 1; else kind = 2;
+    if (P.implicit) {                                                  // W3
+      const double snc = st - sc;
+      if (snc > 0.0) { p.wgt = p.wgt * (snc / st); kind = (blk_odd(sb) * snc < ss) ? 0 : 2; }
+      else kind = 1;
+    }
     nu = P.nuc_nu[nuc]; child_src = nuc;
-    if (kind == 0) { scatter_ce(seed, gen, p, P.A[nuc]); return true; }
+    if (kind == 0) { scatter_ce(seed, gen, p, P.A[nuc]); return ev_closeout(P, R, acc, p); }
   }
   if (kind == 1) { record_death(acc, R, p, TDR_T_NABS); return false; }
   double nu_eff = R.kmode ? nu / R.k_prev : nu;
@@ -290,17 +323,25 @@ __device__ __forceinline__ bool ev_surface(const DevProb &P, const DevRun &R, Bl
   const double u0 = p.u, v0 = p.v, w0 = p.w;
   int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
   bool moved_xy = false, moved_z = false;
-  if (flags & F_DX) {
-    if (u0 > 0.0) { p.x = P.xp[p.ix + 1]; if (p.ix + 1 == P.nx) { if (P.bc[1]) p.u = -u0; else { alive = false; atomicAdd(&acc->leak[1], 1u); } } else { p.ix += 1; moved_xy = true; } }
-    else { p.x = P.xp[p.ix]; if (p.ix == 0) { if (P.bc[0]) p.u = -u0; else { alive = false; atomicAdd(&acc->leak[0], 1u); } } else { p.ix -= 1; moved_xy = true; } }
-  }
-  if (flags & F_DY) {
-    if (v0 > 0.0) { p.y = P.yp[p.iy + 1]; if (p.iy + 1 == P.ny) { if (P.bc[3]) p.v = -v0; else { alive = false; atomicAdd(&acc->leak[3], 1u); } } else { p.iy += 1; moved_xy = true; } }
-    else { p.y = P.yp[p.iy]; if (p.iy == 0) { if (P.bc[2]) p.v = -v0; else { alive = false; atomicAdd(&acc->leak[2], 1u); } } else { p.iy -= 1; moved_xy = true; } }
-  }
-  if (flags & F_DZ) {
-    if (w0 > 0.0) { p.z = P.zp[p.iz + 1]; if (p.iz + 1 == P.nz) { if (P.bc[5]) p.w = -w0; else { alive = false; atomicAdd(&acc->leak[5], 1u); } } else { p.iz += 1; moved_z = true; } }
-    else { p.z = P.zp[p.iz]; if (p.iz == 0) { if (P.bc[4]) p.w = -w0; else { alive = false; atomicAdd(&acc->leak[4], 1u); } } else { p.iz -= 1; moved_z = true; } }
+  // lattice / zone planes: the lanes of a warp cross different axes in different directions, so ONE pass handles whichever
+  // axis a lane crossed with selected operands (a second pass only for a lane that crossed two planes at once, G5)
+  for (u32 af = flags & (F_DX | F_DY | F_DZ); af; af &= af - 1) {
+    const int a = (af & F_DX) ? 0 : (af & F_DY) ? 1 : 2;
+    const double c0 = a == 0 ? u0 : a == 1 ? v0 : w0;
+    const double *pl = a == 0 ? P.xp : a == 1 ? P.yp : P.zp;
+    const int n = a == 0 ? P.nx : a == 1 ? P.ny : P.nz;
+    int idx = a == 0 ? p.ix : a == 1 ? p.iy : p.iz;
+    const bool pos = c0 > 0.0;
+    const double plane = pl[idx + (pos ? 1 : 0)];
+    const bool edge = pos ? (idx + 1 == n) : (idx == 0);
+    double cn = c0;
+    if (edge) {
+      const int face = 2 * a + (pos ? 1 : 0);
+      if (P.bc[face]) cn = -c0; else { alive = false; atomicAdd(&acc->leak[face], 1u); }
+    } else idx += pos ? 1 : -1;
+    if (a == 0) { p.x = plane; p.u = cn; p.ix = idx; moved_xy = moved_xy || !edge; }
+    else if (a == 1) { p.y = plane; p.v = cn; p.iy = idx; moved_xy = moved_xy || !edge; }
+    else { p.z = plane; p.w = cn; p.iz = idx; moved_z = moved_z || !edge; }
   }
   if (flags & F_DOUT) p.ring += 1;
   if (flags & F_DIN) p.ring -= 1;
@@ -309,11 +350,21 @@ __device__ __forceinline__ bool ev_surface(const DevProb &P, const DevRun &R, Bl
     if (moved_xy) p.ring = P.univ_nr[nu2];
     else if (nu2 != univ) p.ring = locate_ring(P, nu2, p.x - P.cx[p.ix], p.y - P.cy[p.iy]);
   }
-  if (flags & F_MX) { if (u0 > 0.0) { p.x = P.mesh[0][p.mx + 1]; if (p.mx + 1 < P.mesh_n[0]) p.mx += 1; } else { p.x = P.mesh[0][p.mx]; if (p.mx > 0) p.mx -= 1; } }
-  if (flags & F_MY) { if (v0 > 0.0) { p.y = P.mesh[1][p.my + 1]; if (p.my + 1 < P.mesh_n[1]) p.my += 1; } else { p.y = P.mesh[1][p.my]; if (p.my > 0) p.my -= 1; } }
-  if (flags & F_MZ) { if (w0 > 0.0) { p.z = P.mesh[2][p.mz + 1]; if (p.mz + 1 < P.mesh_n[2]) p.mz += 1; } else { p.z = P.mesh[2][p.mz]; if (p.mz > 0) p.mz -= 1; } }
+  for (u32 mf = flags & (F_MX | F_MY | F_MZ); mf; mf &= mf - 1) {      // mesh planes, the same way (indices clamp at the mesh box)
+    const int a = (mf & F_MX) ? 0 : (mf & F_MY) ? 1 : 2;
+    const double c0 = a == 0 ? u0 : a == 1 ? v0 : w0;
+    int idx = a == 0 ? p.mx : a == 1 ? p.my : p.mz;
+    const bool pos = c0 > 0.0;
+    const double plane = P.mesh[a][idx + (pos ? 1 : 0)];
+    if (pos) { if (idx + 1 < P.mesh_n[a]) idx += 1; } else if (idx > 0) idx -= 1;
+    if (a == 0) { p.x = plane; p.mx = idx; } else if (a == 1) { p.y = plane; p.my = idx; } else { p.z = plane; p.mz = idx; }
+  }
   if (!alive) record_death(acc, R, p, TDR_T_NLEAK);
-  return alive;
+  if (flags & F_TIME) {                                                // TD3: a time edge; the last one is the census
+    p.t = P.t_edges[p.it + 1]; p.it += 1;
+    if (p.it == P.n_t && alive) { alive = false; record_death(acc, R, p, TDR_T_NCENSUS); }
+  }
+  return alive ? ev_closeout(P, R, acc, p) : false;
 }
 
 // ---------------------------------------------------------------------------------- B birth (A1 SOURCE)
@@ -335,6 +386,7 @@ __device__ __forceinline__ void birth_common(const DevProb &P, const double *mg,
 template <bool CE>
 __device__ TDR_COLD void birth_primary(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, u64 i) {
   p.id = i + R.id_offset; p.depth = 0;         // id_offset: this GPU's share of a source sharded by contiguous id ranges
+  p.it = 0; p.t = P.n_t > 0 ? P.t_edges[0] : 0.0; p.wgt = 1.0;         // TD5, W1
   if (P.src_kind == 0) { p.x = P.src_lo[0]; p.y = P.src_lo[1]; p.z = P.src_lo[2]; }
   else {
     Blk b0 = rng_block(R.seed, p.id, R.gen, 0, PUR_POS, 0), b1 = rng_block(R.seed, p.id, R.gen, 0, PUR_POS, 1);
@@ -350,8 +402,8 @@ __device__ TDR_COLD void birth_primary(const DevProb &P, const double *mg, const
 }
 
 template <bool CE>
-__device__ TDR_COLD void birth_site(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, const tdr_site &s) {
-  p.id = s.id; p.depth = s.depth; p.x = s.x; p.y = s.y; p.z = s.z;
+__device__ TDR_COLD void birth_site(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p, const tdr_site &s, double t = 0.0, double wgt = 1.0) {
+  p.id = s.id; p.depth = s.depth; p.x = s.x; p.y = s.y; p.z = s.z; p.t = t; p.it = s.it; p.wgt = wgt;
   p.ix = s.ix; p.iy = s.iy; p.iz = s.iz; p.mx = s.mx; p.my = s.my; p.mz = s.mz; p.ring = s.ring;
   birth_common<CE>(P, mg, R, acc, p, s.src, true);
 }
@@ -360,6 +412,6 @@ __device__ __forceinline__ tdr_site make_site(const DevRun &R, const Part &p, in
   tdr_site s;
   s.x = p.x; s.y = p.y; s.z = p.z; s.id = derive_id(R.seed, p.id, R.gen, p.seg, c);
   s.ix = (short)p.ix; s.iy = (short)p.iy; s.iz = (short)p.iz; s.mx = (short)p.mx; s.my = (short)p.my; s.mz = (short)p.mz;
-  s.ring = (unsigned char)p.ring; s.src = (unsigned char)src; s.depth = (unsigned char)(R.kmode ? 0 : p.depth + 1); s.pad = 0;
+  s.ring = (unsigned char)p.ring; s.src = (unsigned char)src; s.depth = (unsigned char)(R.kmode ? 0 : p.depth + 1); s.it = (unsigned char)p.it;
   return s;
 }

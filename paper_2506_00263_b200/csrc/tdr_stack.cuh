@@ -45,11 +45,11 @@ __device__ TDR_COLD void push_children(const DevOut &O, const DevRun &R, BlockAc
     u64 t = base + excl + c;
     tdr_site s = make_site(R, p, src, (u32)c);
     if (R.kmode) { if (t < R.bank_cap) R.bank[t] = s; else atomicExch(O.err, TDR_ECAPACITY); }
-    else if (!R.sec_flag) { if (t - R.sec_head0 < R.sec_cap) R.sec[t % R.sec_cap] = s; else atomicExch(O.err, TDR_ECAPACITY); }
+    else if (!R.sec_flag) { if (t - R.sec_head0 < R.sec_cap) { R.sec[t % R.sec_cap] = s; if (R.sec_time) R.sec_time[t % R.sec_cap] = p.t; if (R.sec_w) R.sec_w[t % R.sec_cap] = p.wgt; } else atomicExch(O.err, TDR_ECAPACITY); }
     else {                                                       // asynchronous scheme: publish with a ready flag
       const u64 k = t % R.sec_cap;
       if ((i64)(t - *(const volatile u64 *)R.sec_head) < (i64)(R.sec_cap - SEC_MARGIN)) {     // the head may already be past t
-        R.sec[k] = s; __threadfence(); *(volatile u64 *)&R.sec_flag[k] = t + 1;
+        R.sec[k] = s; if (R.sec_time) R.sec_time[k] = p.t; if (R.sec_w) R.sec_w[k] = p.wgt; __threadfence(); *(volatile u64 *)&R.sec_flag[k] = t + 1;
       } else atomicExch(O.err, TDR_ECAPACITY);
     }
   }
@@ -68,7 +68,7 @@ __device__ __forceinline__ bool make_work(const DevProb &P, const double *mg, co
       h = __shfl_sync(FULL, h, leader);
       if (dead && h != ~0ull) {
         u64 idx = h + __popc(m & lanemask_lt());
-        if (idx < R.sec_limit) { tdr_site s = R.sec[idx % R.sec_cap]; birth_site<CE>(P, mg, R, acc, p, s); reborn = true; }
+        if (idx < R.sec_limit) { tdr_site s = R.sec[idx % R.sec_cap]; birth_site<CE>(P, mg, R, acc, p, s, R.sec_time ? R.sec_time[idx % R.sec_cap] : 0.0, R.sec_w ? R.sec_w[idx % R.sec_cap] : 1.0); reborn = true; }
       }
     }
   }
@@ -109,7 +109,7 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
   acc_init(&acc);
   for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (u64)gridDim.x * blockDim.x) {
     Part p;
-    if (i < n_sec) { tdr_site s = R.sec[(sec_start + i) % R.sec_cap]; birth_site<CE>(P, mg, R, &acc, p, s); }
+    if (i < n_sec) { tdr_site s = R.sec[(sec_start + i) % R.sec_cap]; birth_site<CE>(P, mg, R, &acc, p, s, R.sec_time ? R.sec_time[(sec_start + i) % R.sec_cap] : 0.0, R.sec_w ? R.sec_w[(sec_start + i) % R.sec_cap] : 1.0); }
     else {
       u64 idx = src_start + (i - n_sec);
       if (R.src_sites) { tdr_site s = R.sites[idx]; birth_site<CE>(P, mg, R, &acc, p, s); }
@@ -159,7 +159,7 @@ __global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa
         else if (flags & F_COLLIDE) {
           if (HYBRID) {
             if (k > 0) store_part<CE>(S, slot, p);       // an earlier crossing of this launch changed direction / indices too
-            else { S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; }
+            else { S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; if (S.t) S.t[slot] = p.t; }
             S.s_sigt[slot] = St;
             if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
             to_collide = true; alive = false;
@@ -242,6 +242,13 @@ __global__ void __launch_bounds__(256) k_popctrl(const tdr_site *bank, u64 n_ban
       if (base + r < next_cap) next[base + r] = s; else atomicExch(err, TDR_ECAPACITY);
     }
   }
+}
+
+// N5 for tallies too large to be block-private (global `red`): after every generation / run, a bin whose top bit is set
+// has left int64 (scores are non-negative; one generation cannot add 2^63 to a bin)
+__global__ void k_overflow_check(const u64 *flux, const u64 *coll, u64 n_bins, int *err) {
+  for (u64 i = (u64)blockIdx.x * blockDim.x + threadIdx.x; i < n_bins; i += (u64)gridDim.x * blockDim.x)
+    if ((flux[i] | coll[i]) >> 63) atomicExch(err, TDR_EOVERFLOW);
 }
 
 // ---------------------------------------------------------------------------------- unit kernels

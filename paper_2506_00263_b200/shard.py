@@ -38,7 +38,7 @@ def run_fixed_source_sharded(problem, n, seed, rank, world, device, **options):
         P.close()
 
 
-def run_k_eigenvalue_shares(engines, shares, n, n_inactive, n_active, seed, allreduce4=None):
+def run_k_eigenvalue_shares(engines, shares, n, n_inactive, n_active, seed, allreduce4=None, read=True):
     """ONE k-eigenvalue problem of n particles per generation (D2 in steps, include/tdr.h).  `engines` are the shares this
     process drives — one per process under torch.distributed, or several in turn on one GPU — and `shares` their
     (rank, world) pairs.  An engine offers k_begin / k_generation / k_population_control / k_end / scale / read_tallies
@@ -74,14 +74,14 @@ def run_k_eigenvalue_shares(engines, shares, n, n_inactive, n_active, seed, allr
     out = []
     for e in engines:
         e.k_end(n_inactive, gen_n, gen_m, gen_p, gen_pc, gen_k)
-        out.append(e.read_tallies(history=False, bank=True))
+        out.append(e.read_tallies(history=False, bank=True) if read else None)
     return out
 
 
-def run_k_eigenvalue_sharded(engine, n, n_inactive, n_active, seed, rank, world):
+def run_k_eigenvalue_sharded(engine, n, n_inactive, n_active, seed, rank, world, read=True):
     """This rank's share of one k-eigenvalue problem under torch.distributed (one process per GPU)."""
     return run_k_eigenvalue_shares([engine], [(rank, world)], n, n_inactive, n_active, seed,
-                                   allreduce4=allreduce_int64 if world > 1 else None)[0]
+                                   allreduce4=allreduce_int64 if world > 1 else None, read=read)[0]
 
 
 def allreduce_int64(vals, group=None):

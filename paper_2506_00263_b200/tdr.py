@@ -10,12 +10,12 @@ import numpy as np
 
 from . import build as _build
 
-MAX_RINGS, MAX_NUC, T_COUNT = 4, 4, 12
+MAX_RINGS, MAX_NUC, T_COUNT = 4, 4, 16
 TOTAL_NAMES = ["n_seg", "n_coll", "n_cross", "n_abs", "n_fis", "n_leak", "n_born", "n_dropped",
-               "n_dirfail", "digest", "n_sites"]
+               "n_dirfail", "digest", "n_sites", "n_census", "n_roulette"]
 SITE_DTYPE = np.dtype([("x", "<f8"), ("y", "<f8"), ("z", "<f8"), ("id", "<u8"), ("ix", "<i2"), ("iy", "<i2"),
                        ("iz", "<i2"), ("mx", "<i2"), ("my", "<i2"), ("mz", "<i2"), ("ring", "u1"),
-                       ("src", "u1"), ("depth", "u1"), ("pad", "u1")])
+                       ("src", "u1"), ("depth", "u1"), ("it", "u1")])
 PD, PI = C.POINTER(C.c_double), C.POINTER(C.c_int32)
 
 
@@ -28,12 +28,13 @@ class tdr_geometry(C.Structure):
                 ("src_kind", C.c_int32), ("src_lo", C.c_double * 3), ("src_hi", C.c_double * 3),
                 ("src_dir_kind", C.c_int32), ("src_dir", C.c_double * 3),
                 ("src_energy_kind", C.c_int32), ("src_index", C.c_int32), ("src_energy", C.c_double),
-                ("tally_scale_log2", C.c_int32)]
+                ("tally_scale_log2", C.c_int32), ("n_tbins", C.c_int32), ("t_edges", PD),
+                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double)]
 
 
 class tdr_materials(C.Structure):
     _fields_ = [("n_mat", C.c_int32), ("G", C.c_int32), ("sig_t", PD), ("sig_s", PD), ("sig_f", PD), ("nu", PD),
-                ("chi", PD), ("mat_nnuc", PI), ("mat_nuc", PI), ("mat_dens", PD)]
+                ("chi", PD), ("mat_nnuc", PI), ("mat_nuc", PI), ("mat_dens", PD), ("speed", PD)]
 
 
 class tdr_xs_tables(C.Structure):
@@ -60,7 +61,7 @@ class tdr_diag(C.Structure):
 
 EXPORTS = ["tdr_init_problem", "tdr_set_option", "tdr_workspace_bytes", "tdr_bind_workspace", "tdr_run_fixed_source",
            "tdr_run_k_eigenvalue", "tdr_tally_sizes", "tdr_read_tallies", "tdr_read_diagnostics", "tdr_free_problem",
-           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw", "tdr_k_begin", "tdr_k_generation", "tdr_k_population_control", "tdr_k_end"]
+           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw", "tdr_k_begin", "tdr_k_generation", "tdr_k_population_control", "tdr_k_end", "tdr_measure_peak"]
 
 _lib = None
 
@@ -81,6 +82,7 @@ def lib():
         L.tdr_k_generation.argtypes = [C.c_void_p, C.c_uint32, C.c_int, C.c_double, C.c_int, C.POINTER(C.c_int64)]
         L.tdr_k_population_control.argtypes = [C.c_void_p, C.c_uint32, C.c_double, C.POINTER(C.c_uint64)]
         L.tdr_k_end.argtypes = [C.c_void_p, C.c_uint32, C.c_uint32, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.tdr_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.c_void_p]
         L.tdr_tally_sizes.argtypes = [C.c_void_p, C.POINTER(tdr_sizes)]
         L.tdr_read_tallies.argtypes = [C.c_void_p, C.POINTER(tdr_tallies)]
         L.tdr_read_diagnostics.argtypes = [C.c_void_p, C.POINTER(tdr_diag)]
@@ -248,3 +250,11 @@ def dev_draw(seed, ids, gen, seg, purpose, j):
     out = torch.empty(ids.numel(), dtype=torch.float64, device=ids.device)
     _check(lib().tdr_dev_draw(seed, ids.data_ptr(), gen, seg, purpose, j, out.data_ptr(), ids.numel(), torch.cuda.current_stream().cuda_stream), "tdr_dev_draw")
     return out
+
+
+def measure_peak(what):
+    """what: "fp64" -> DFMA TFLOP/s, "l2" -> L2-resident copy GB/s, measured on the current device by the library's micro-benchmarks."""
+    import torch
+    v = C.c_double()
+    _check(lib().tdr_measure_peak({"fp64": 0, "l2": 1}[what], C.byref(v), torch.cuda.current_stream().cuda_stream), "tdr_measure_peak")
+    return v.value

@@ -44,7 +44,7 @@ def _i32(a):
 
 def geometry(xplanes, yplanes, zplanes, cell_univ, universes, bc, mesh=None, by_group=0,
              e_edges=None, src_kind=0, src_lo=(0, 0, 0), src_hi=(0, 0, 0), src_dir=None,
-             src_energy=("group", 0), scale_log2=24, cx=None, cy=None):
+             src_energy=("group", 0), scale_log2=24, cx=None, cy=None, t_edges=None, implicit=None):
     """universes: list of (radii ascending, materials innermost..background)."""
     xp, yp, zp = _f64(xplanes), _f64(yplanes), _f64(zplanes)
     nx, ny, nz = len(xp) - 1, len(yp) - 1, len(zp) - 1
@@ -74,15 +74,21 @@ def geometry(xplanes, yplanes, zplanes, cell_univ, universes, bc, mesh=None, by_
              src_energy_kind=ekind,
              src_index=int(src_energy[1]) if ekind != 1 else 0,
              src_energy=float(src_energy[1]) if ekind == 1 else 0.0,
-             tally_scale_log2=int(scale_log2))
+             tally_scale_log2=int(scale_log2),
+             n_tbins=(len(t_edges) - 1 if t_edges is not None else 0), t_edges=_f64(t_edges if t_edges is not None else [0.0]),
+             implicit_capture=0 if implicit is None else 1, w_roulette=0.0 if implicit is None else float(implicit[0]),
+             w_survive=0.0 if implicit is None else float(implicit[1]))
     return g
 
 
-def mg_materials(sig_t, sig_s, sig_f, nu, chi):
+def mg_materials(sig_t, sig_s, sig_f, nu, chi, speed=None):
     sig_t = _f64(sig_t)
     n_mat, G = sig_t.shape
-    return dict(n_mat=n_mat, G=G, sig_t=sig_t, sig_s=_f64(sig_s).reshape(n_mat, G, G), sig_f=_f64(sig_f).reshape(n_mat, G),
-                nu=_f64(nu).reshape(n_mat, G), chi=_f64(chi).reshape(n_mat, G))
+    d = dict(n_mat=n_mat, G=G, sig_t=sig_t, sig_s=_f64(sig_s).reshape(n_mat, G, G), sig_f=_f64(sig_f).reshape(n_mat, G),
+             nu=_f64(nu).reshape(n_mat, G), chi=_f64(chi).reshape(n_mat, G))
+    if speed is not None:
+        d["speed"] = _f64(speed).reshape(G)                  # time-dependent runs: speed of each group
+    return d
 
 
 def ce_materials(mats):
@@ -212,6 +218,41 @@ def ce_lerp_absorber(E0, n=100000, seed=1):
     geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, e_edges=[1e-3, 1e5],
                    src_energy=("mono", E0))
     return Problem("ce_lerp_absorber", geo, ce_materials([[(0, 0.4)]]), xs, "fixed", n, seed=seed)
+
+
+def td_medium(sig_t, sig_s, speed, t_edges, sig_f=0.0, nu=0.0, n=100000, seed=1):
+    """Time-dependent pin: one-group infinite medium, point source at t_edges[0], time-mesh tally, census at
+    t_edges[-1].  With removal rate S_a v the population is N(t) = exp(-S_a v t) (k_inf = 0), so the track length in a time
+    bin and the census fraction have closed forms."""
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, t_edges=t_edges)
+    mats = mg_materials([[sig_t]], [[[sig_s]]], [[sig_f]], [[nu]], [[1.0]], speed=[speed])
+    return Problem("td_medium", geo, mats, None, "fixed", n, seed=seed)
+
+
+def td_ce_absorber(E0, t_edges, n=100000, seed=1):
+    """Continuous-energy pure absorber (sigma_c = 2 b flat, N = 0.5), mono-energetic source: pins the speed law v(E)."""
+    xs = dict(n_grid=4, n_nuc=1, energy=_f64([1e-5, 1.0, 1e3, 2e7]), A=_f64([10.0]), sig_s=_f64(np.zeros((1, 4))),
+              sig_c=_f64(np.full((1, 4), 2.0)), sig_f=_f64(np.zeros((1, 4))), nu=_f64([0.0]), watt_a=_f64([1.0]), watt_b=_f64([1.0]))
+    geo = geometry([-INF, INF], [-INF, INF], [-INF, INF], [0], [((), (0,))], [0] * 6, e_edges=[1e-5, 2e7],
+                   src_energy=("mono", E0), t_edges=t_edges)
+    return Problem("td_ce_absorber", geo, ce_materials([[(0, 0.5)]]), xs, "fixed", n, seed=seed)
+
+
+def cfg3_td(n=1000000, n_tbins=128, t_max=3.0e-6, seed=1, n_grid=50000, sigf0=None):
+    """The paper's own continuous-energy experiment: the infinite pin cell with a uniform 14 MeV source
+    at t = 0, a time-mesh tally of 1 ... 128 bins and a census at t_max.  One energy bin."""
+    geo, mats, xs = _ce_pin(1, n_grid, ("mono", 14e6), CE_SIGF0 if sigf0 is None else sigf0)
+    geo["n_tbins"] = int(n_tbins)
+    geo["t_edges"] = _f64(np.linspace(0.0, t_max, n_tbins + 1))
+    return Problem("cfg3_td", geo, mats, xs, "fixed", n, seed=seed)
+
+
+def with_implicit_capture(problem, w_roulette=0.25, w_survive=0.5):
+    """The same fixed-source problem with implicit capture and weight roulette (readings W1-W4)."""
+    assert problem.mode == "fixed"
+    problem.geometry.update(implicit_capture=1, w_roulette=float(w_roulette), w_survive=float(w_survive))
+    problem.name += "_ic"
+    return problem
 
 
 def _mg_material(rng, G, kind):

@@ -19,10 +19,33 @@ def assert_same(o, g, what=""):
         assert np.array_equal(np.sort(o["bank"].view(np.dtype((np.void, 48)))), np.sort(g["bank"].view(np.dtype((np.void, 48))))), (what, "bank multiset")
 
 
-def run_both(problem, **options):
+_ORACLE_CACHE = {}
+
+
+def _problem_key(p):
+    import hashlib
+    h = hashlib.sha1()
+    for d in (p.geometry, p.materials, p.xs or {}):
+        for k in sorted(d):
+            v = d[k]
+            h.update(k.encode()); h.update(np.ascontiguousarray(v).tobytes() if isinstance(v, np.ndarray) else repr(v).encode())
+    return (p.mode, p.n_particles, p.n_inactive, p.n_active, p.seed, h.hexdigest())
+
+
+def oracle_result(problem):
+    """The oracle's result for this problem, computed once per test session (many variants are compared with the same run)."""
     from oracle import orc
+    k = _problem_key(problem)
+    if k not in _ORACLE_CACHE:
+        if len(_ORACLE_CACHE) > 24:
+            _ORACLE_CACHE.pop(next(iter(_ORACLE_CACHE)))
+        _ORACLE_CACHE[k] = orc.run(problem)
+    return _ORACLE_CACHE[k]
+
+
+def run_both(problem, **options):
     from paper_2506_00263_b200 import tdr
-    o = orc.run(problem)
+    o = oracle_result(problem)
     P = tdr.Problem(problem, **options)
     try:
         g = P.run()

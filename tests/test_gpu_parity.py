@@ -266,3 +266,83 @@ def test_k_eigenvalue_in_three_shares_equals_the_unsharded_oracle(scheme):
         assert np.array_equal(parts[0]["gen_k"], o["gen_k"]) and parts[1]["k_mean"] == o["k_mean"]
         bank = np.concatenate([x["bank"] for x in parts])
         assert np.array_equal(np.sort(bank.view(np.dtype((np.void, 48)))), np.sort(o["bank"].view(np.dtype((np.void, 48)))))
+
+
+# ------------------------------------------------------------------ time-dependent fixed source
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+def test_time_dependent_fixed_source_parity(scheme, decomp):
+    """Time in the particle state, the time-edge candidate distance, the time-mesh tally and the census, on all six
+    scheme x decomposition variants: the continuous-energy pin cell of the paper's experiment at three mesh widths, and the
+    one-group media with closed forms (pure absorber, scatterer, supercritical chain whose secondaries inherit the time)."""
+    probs = [W.cfg3_td(n=8009, n_tbins=nt) for nt in (1, 16, 128)]
+    probs += [W.td_medium(1.0, 0.0, 2.5, [0.0, 0.05, 0.2, 0.21, 0.5, 0.9, 1.2], n=20011),
+              W.td_medium(1.0, 0.7, 2.5, [0.0, 0.3, 1.2], n=20011),
+              W.td_medium(1.0, 0.5, 1.0, np.linspace(0.0, 3.0, 7), sig_f=0.3, nu=2.5, n=5003),
+              W.td_ce_absorber(0.0253, np.linspace(0.0, 4.5e-6, 5), n=10007)]
+    for p in probs:
+        o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+        assert_same(o, g, f"{p.name}/{scheme}/{decomp}")
+        assert g["totals"]["n_census"] > 0 and g["totals"]["n_census"] == o["totals"]["n_census"]
+    # a small window forces refills and, under the stack scheme, the secondary ring with its parallel time array
+    p = W.cfg3_td(n=5003, n_tbins=8)
+    o, g, _ = run_both(p, scheme=scheme, decomposition=decomp, window=1024)
+    assert_same(o, g, "cfg3_td/window=1024")
+
+
+def test_time_dependent_full_size_and_closed_form_on_gpu():
+    from paper_2506_00263_b200 import tdr
+    for scheme in ("stack", "async"):
+        o, g, _ = run_both(W.cfg3_td(n=1000000, n_tbins=128), scheme=scheme)
+        assert_same(o, g, f"cfg3_td full size/{scheme}")
+    # N(t) = exp(-S_a v t) straight from the CUDA path
+    n, edges = 200000, np.array([0.0, 0.05, 0.2, 0.21, 0.5, 0.9, 1.2])
+    P = tdr.Problem(W.td_medium(1.0, 0.7, 2.5, edges, n=n))
+    g = P.run(); P.close()
+    ref = -np.diff(np.exp(-0.3 * 2.5 * edges)) / 0.3
+    assert np.all(np.abs(g["flux"] / 2 ** 24 / n - ref) < 4 * np.sqrt(np.diff(edges) * 2.5 * ref / n) + 1e-7)
+    # particle stashes refuse a time mesh loudly; k-mode refuses it too
+    with pytest.raises(tdr.TdrError):
+        tdr.Problem(W.cfg3_td(n=1000, n_tbins=4), scheme="async", stash="shared").run()
+
+
+def test_tally_overflow_is_reported():
+    """N5 / TDR_EOVERFLOW (-6): a fixed-point sum that leaves int64 is an error on both sides, never a silent wrap."""
+    from oracle import orc
+    from paper_2506_00263_b200 import tdr
+    p = W.infinite_medium([1e-4], [[0.0]], n=100000)
+    p.geometry["tally_scale_log2"] = 40                       # 1e5 histories x 1e4 cm x 2^40 = 1.1e21 > 2^63
+    with pytest.raises(RuntimeError, match="-6"):
+        orc.run(p)
+    for scheme in ("stack", "async"):
+        P = tdr.Problem(p, scheme=scheme)
+        with pytest.raises(tdr.TdrError) as e:
+            P.run()
+        assert e.value.code == -6, e.value
+        P.close()
+    # a mesh tally too large to be block-private: the per-run scan of the bins
+    q = W.slab_mesh(1e-4, 0.0, 2.0e5, mesh=list(np.linspace(0.0, 2.0e5, 301)), n=200000)
+    q.geometry["tally_scale_log2"] = 40                       # ~660 cm per bin and history x 2e5 x 2^40 = 1.4e20
+    for scheme in ("stack", "async"):
+        P = tdr.Problem(q, scheme=scheme)
+        with pytest.raises(tdr.TdrError) as e:
+            P.run()
+        assert e.value.code == -6, e.value
+        P.close()
+
+
+# ------------------------------------------------------------------ implicit capture + weight roulette (SURVEY 8f-2; PAPER.md:121 closeout)
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+def test_implicit_capture_and_roulette_parity(scheme, decomp):
+    """Weights in the state, weighted scores, capture by weight reduction and the closeout's roulette, on all six
+    scheme x decomposition variants, multigroup and continuous energy, with fission secondaries that inherit the weight,
+    and together with the time mesh."""
+    ic = W.with_implicit_capture
+    probs = [ic(W.cfg0(n=20011)), ic(W.slab_mesh(1.0, 0.8, 2.0, lattice=[0.5, 1.25], mesh=[0.0, 0.11, 0.4, 0.75, 1.0, 1.31, 1.9, 2.0], n=20011), 0.1, 0.3),
+             ic(W.infinite_medium([1.0], [[0.5]], [0.2], [1.5], mode="fixed", n=10007)), ic(W.ce_two_nuclide_medium(mode="fixed", n=5003)),
+             ic(W.cfg3(n=8009, n_ebins=100)), ic(W.cfg3_td(n=5003, n_tbins=16)), ic(W.two_region("lattice", n=10007), 0.3, 0.9)]
+    for p in probs:
+        o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+        assert_same(o, g, f"{p.name}/{scheme}/{decomp}")
+        assert g["totals"]["n_roulette"] > 0 and g["totals"]["n_abs"] == 0
+    o, g, _ = run_both(ic(W.cfg3(n=5003, n_ebins=1)), scheme=scheme, decomposition=decomp, window=1024)
+    assert_same(o, g, "cfg3_ic/window=1024")

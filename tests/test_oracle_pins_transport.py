@@ -380,3 +380,121 @@ def test_population_control_ids_are_distinct_and_population_is_unbiased():
     assert len(np.unique(r["hist_id"])) == len(r["hist_id"]) == int(r["gen_n"][-1])
     assert np.all(np.abs(r["gen_n"].astype(float) - 30000) < 4 * math.sqrt(30000 * 0.25) + 1)
     assert len(np.unique(r["bank"]["id"])) == len(r["bank"])
+
+
+# ------------------------------------------------------------------ TD: time-dependent fixed source
+@pytest.mark.parametrize("c", [0.0, 0.7])
+def test_time_dependent_population_decays_exponentially(c):
+    """One-group infinite medium, speed v: collisions do not change the speed, so the population is N(t) = exp(-S_a v t)
+    whatever the scattering ratio.  Track length per source in the time bin [a, b] = (exp(-S_a v a) - exp(-S_a v b)) / S_a,
+    the census fraction is exp(-S_a v t_max).  Pins the time advance, the time-edge candidate, the time-bin index and census."""
+    St, v, n = 1.0, 2.5, 200000
+    Sa = St * (1 - c)
+    edges = np.array([0.0, 0.05, 0.2, 0.21, 0.5, 0.9, 1.2])
+    r = orc.run(W.td_medium(St, c * St, v, edges, n=n))
+    T = r["totals"]
+    ref = -np.diff(np.exp(-Sa * v * edges)) / Sa
+    got = r["flux"] / S24 / n
+    assert np.all(np.abs(got - ref) < 4 * np.sqrt(np.diff(edges) * v * ref / n) + 1e-7), (got, ref)
+    surv = math.exp(-Sa * v * edges[-1])
+    assert abs(T["n_census"] / n - surv) < 4 * math.sqrt(surv * (1 - surv) / n)
+    assert T["n_born"] == T["n_abs"] + T["n_census"] == n and T["n_leak"] == 0
+    assert abs(r["coll"].sum() / S24 / n - St * ref.sum()) < 4 * math.sqrt(3 * St * ref.sum() / n)
+
+
+def test_time_dependent_fission_chain_growth():
+    """Supercritical medium: the expected population grows as exp((nu S_f - S_a) v t); the census count pins secondaries that
+    inherit their parent's time (a child restarted at t = 0 would never reach the census in time)."""
+    St, Ss, Sf, nu, v, n = 1.0, 0.5, 0.3, 2.5, 1.0, 100000
+    Sa = St - Ss
+    alpha = (nu * Sf - Sa) * v
+    edges = np.linspace(0.0, 3.0, 7)
+    r = orc.run(W.td_medium(St, Ss, v, edges, sig_f=Sf, nu=nu, n=n))
+    T = r["totals"]
+    grow = math.exp(alpha * edges[-1])
+    assert abs(T["n_census"] / n - grow) < 0.03 * grow                     # branching-process variance: a few sigma at 1e5
+    ref = np.diff(np.exp(alpha * edges)) / alpha * v                        # integral of N(t) v dt per bin
+    got = r["flux"] / S24 / n
+    assert np.all(np.abs(got / ref - 1) < 0.03), (got, ref)
+    assert T["n_born"] == n + T["n_sites"] == T["n_abs"] + T["n_fis"] + T["n_census"]
+
+
+@pytest.mark.parametrize("E0", [0.0253, 1.0e6])
+def test_time_dependent_speed_law_of_continuous_energy(E0):
+    """v = 1.3831592e6 cm/s x sqrt(E / eV) (TD1): 2200 m/s at 0.0253 eV.  In a flat pure absorber the census fraction at
+    t_max is exp(-S v t_max); t_max is set to one mean lifetime 1 / (S v) with v from the textbook value."""
+    v = 2.19991e5 if E0 == 0.0253 else 1.3831592e9
+    S = 0.5 * 2.0
+    tmax = 1.0 / (S * v)
+    edges = np.linspace(0.0, tmax, 5)
+    n = 100000
+    r = orc.run(W.td_ce_absorber(E0, edges, n=n))
+    surv = math.exp(-1.0)
+    assert abs(r["totals"]["n_census"] / n - surv) < 4 * math.sqrt(surv * (1 - surv) / n) + 2e-4
+    ref = -np.diff(np.exp(-S * v * edges)) / S
+    assert np.all(np.abs(r["flux"] / S24 / n - ref) < 4 * np.sqrt(ref * ref / n) + 1e-3 * ref)
+
+
+def test_time_mesh_resolution_does_not_change_the_physics():
+    """The paper's sweep: time-mesh widths 1, 2, ... 128.  A finer mesh adds time-edge crossings (each one a
+    segment, so the random streams differ) but must not change any expectation: the summed flux, the collisions and the
+    census of the CE pin cell agree within statistics for every width."""
+    n, out = 20000, []
+    for nt in (1, 8, 128):
+        r = orc.run(W.cfg3_td(n=n, n_tbins=nt, n_grid=4000))
+        T = r["totals"]
+        assert T["n_born"] == T["n_abs"] + T["n_fis"] + T["n_census"] + T["n_leak"] and T["n_census"] > 0
+        assert len(r["flux"]) == nt and int(r["coll"].sum()) == T["n_coll"] << 24
+        out.append((r["flux"].sum() / S24 / n, T["n_coll"] / n, T["n_census"] / n, T["n_born"] / n))
+    for a in out[1:]:
+        assert np.allclose(a, out[0], rtol=0.1), out                   # branching-process noise at 2e4 sources
+
+
+# ------------------------------------------------------------------ W: implicit capture + weight roulette (SURVEY 8f-2)
+def test_implicit_capture_keeps_every_expectation_and_cuts_the_variance():
+    """Capture by weight reduction and roulette below w_roulette change no expectation: flux per source 1 / S_a and
+    collisions per source S_t / S_a in the infinite medium, with nobody captured in the analog way and every history
+    ended by the roulette; the spread over batches is smaller than the analog one."""
+    n = 100000
+    r = orc.run(W.with_implicit_capture(W.cfg0(n=n)))
+    T = r["totals"]
+    assert T["n_abs"] == 0 and T["n_roulette"] == n == T["n_born"]
+    assert abs(r["flux"][0] / S24 / n - 1 / 0.3) < 4 * (1 / 0.3) / math.sqrt(n)
+    assert abs(r["coll"][0] / S24 / n - 1 / 0.3) < 4 * math.sqrt(0.7 / 0.09 / n)
+    o = orc.Oracle(W.cfg0(n=500)); a = np.array([o.run(seed=s)["coll"][0] for s in range(1, 41)]) / S24 / 500; o.close()
+    o = orc.Oracle(W.with_implicit_capture(W.cfg0(n=500))); b = np.array([o.run(seed=s)["coll"][0] for s in range(1, 41)]) / S24 / 500; o.close()
+    assert b.std() < 0.8 * a.std(), (a.std(), b.std())
+
+
+def test_implicit_capture_in_the_scattering_slab_matches_the_integral_equation():
+    """Weighted scores per mesh bin against the deterministic slab solution: the weight after each collision, the scores
+    that carry it and the roulette are all in play; the analog run of the same slab is the second witness."""
+    St, c, Lx, n = 1.0, 0.8, 2.0, 400000
+    mesh = [0.0, 0.11, 0.4, 0.75, 1.0, 1.31, 1.9, 2.0]
+    r = orc.run(W.with_implicit_capture(W.slab_mesh(St, c * St, Lx, lattice=[0.5, 1.25], mesh=mesh, n=n), 0.1, 0.3))
+    x, Ct, T, R = _slab_collision_probability(St, c, Lx)
+    cum = np.concatenate([[0.0], np.cumsum(Ct)])
+    ref_bin = np.diff(np.interp(mesh, x, cum))
+    coll, flux = r["coll"] / S24 / n, r["flux"] / S24 / n
+    assert np.all(np.abs(coll - ref_bin) < 4 * np.sqrt(3 * ref_bin / n)), (coll, ref_bin)
+    assert np.all(np.abs(flux - ref_bin / St) < 4 * np.sqrt(3 * ref_bin / n) / St), (flux, ref_bin / St)
+    assert r["totals"]["n_abs"] == 0 and r["totals"]["n_roulette"] > 0
+    assert r["totals"]["n_born"] == r["totals"]["n_roulette"] + r["totals"]["n_leak"]
+
+
+@pytest.mark.parametrize("ce", [False, True])
+def test_implicit_capture_with_fission_chains(ce):
+    """Fission stays analog under implicit capture (W3) and children inherit the weight (W1): flux per source neutron is
+    1 / (S_a - nu S_f) in a sub-critical infinite medium, multigroup and continuous energy."""
+    n = 100000
+    if ce:
+        p = W.ce_two_nuclide_medium(mode="fixed", n=n)
+        ref = 1.0 / (0.5 * 1.0 + 0.3 * 2.0 - 0.3 * 2.0 * 1.5)
+    else:
+        p = W.infinite_medium([1.0], [[0.5]], [0.2], [1.5], mode="fixed", n=n)
+        ref = 1.0 / (0.5 - 1.5 * 0.2)
+    a = orc.run(p)
+    r = orc.run(W.with_implicit_capture(p))
+    assert abs(r["flux"].sum() / S24 / n - ref) < 0.03 * ref and abs(a["flux"].sum() / S24 / n - ref) < 0.03 * ref
+    T = r["totals"]
+    assert T["n_abs"] == 0 and T["n_born"] == n + T["n_sites"] == T["n_fis"] + T["n_roulette"]
