@@ -209,8 +209,9 @@ def run_reference(args, rank, world):
 
 # ---------------------------------------------------------------------------------------------------- the CUDA path
 class Runner:
-    def __init__(self, rank, world, local_rank):
+    def __init__(self, rank, world, local_rank, extra_opts=None):
         import torch
+        self.extra_opts = dict(extra_opts or {})
         self.torch, self.rank, self.world, self.dev = torch, rank, world, f"cuda:{local_rank}"
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)
         self.prof = profile_metrics()
@@ -244,7 +245,9 @@ class Runner:
         from paper_2506_00263_b200 import tdr
         torch = self.torch
         scheme, decomp, stash = variant
-        opts = dict(scheme=scheme, decomposition=decomp, keep_history=0, **({"stash": stash} if stash else {}))
+        if self.rank == 0:
+            print(f"[bench] {name} {vkey(variant)}: {warmup} warm-up + {steps} timed step(s)", file=sys.stderr, flush=True)
+        opts = dict(scheme=scheme, decomposition=decomp, keep_history=0, **({"stash": stash} if stash else {}), **self.extra_opts)
         P = tdr.Problem(prob, device=self.dev, time_kernels=1, **opts)
         for _ in range(warmup):
             self.run_once(P, prob)
@@ -322,7 +325,7 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
-    R = Runner(rank, world, local_rank)
+    R = Runner(rank, world, local_rank, dict(kv.split("=", 1) for kv in args.opt))
     single = args.workload is not None
     head_name = args.workload or HEADLINE
     head_prob = make_problem(head_name, args.scale)
@@ -348,9 +351,13 @@ def run_ours(args, rank, world, local_rank):
             prob = make_problem(name, args.scale)
             es = {}
             for v in VARIANTS[name]:
-                e, _, _ = R.time_variant(name, prob, v, aux_steps, aux_warm)
+                try:
+                    e, _, _ = R.time_variant(name, prob, v, aux_steps, aux_warm)
+                except Exception as ex:                                # a side variant must not cost the headline its line
+                    e = {"error": f"{type(ex).__name__}: {ex}", "value": 0.0}
                 es[vkey(v)] = e
-            workloads[name] = {"workload": FULL[name]["desc"], "variants": es, "all_variants_bit_identical": len({e["digest"] for e in es.values()}) == 1}
+            workloads[name] = {"workload": FULL[name]["desc"], "variants": es,
+                               "all_variants_bit_identical": len({e.get("digest", e.get("error")) for e in es.values()}) == 1}
     if rank == 0:
         e = head_entry
         best = {n: max(w["variants"], key=lambda k: w["variants"][k]["value"]) for n, w in workloads.items()}
@@ -398,6 +405,7 @@ def main():
     ap.add_argument("--decomposition", default="fused", choices=["fused", "split", "hybrid"])
     ap.add_argument("--stash", default="index", choices=["index", "particle", "shared"])
     ap.add_argument("--scale", type=float, default=1.0, help="scale the particle count of every workload (smoke runs)")
+    ap.add_argument("--opt", action="append", default=[], metavar="KEY=VALUE", help="extra tdr_set_option for every variant timed (sweeps, profiling)")
     ap.add_argument("--headline-only", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-peaks", action="store_true")

@@ -130,15 +130,23 @@ int tdr_init_problem(const tdr_geometry *, const tdr_materials *, const tdr_xs_t
  * "stash_links" (async, links per warp, 8..64); "slots_per_warp" (async); "sync_every" (stack: remap iterations per
  * counter read-back); "blocks_per_sm"; "keep_history" = 0|1; "time_kernels" = 0|1; "idle_timeout_s" (async watchdog);
  * "seg_per_event" (async fused: segments per step event); "seg_per_launch", "drain_below" (stack); "lockstep",
- * "async_threads" (async); "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs).
+ * "async_threads" (async); "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs);
+ * "device_loop" = 1|0 (stack: the remap loop runs as a CUDA-graph WHILE node without the host | host-driven batches of sync_every);
+ * "stash" = auto|index|particle|shared, "pool_slots", "ps_threads" (async: which stash).
  * decomposition = fused (monolithic step) | split (five events) | hybrid (step + collide). */
 int tdr_set_option(tdr_problem *, const char *key, const char *value);
 int tdr_workspace_bytes(const tdr_problem *, uint64_t n_particles, uint64_t *bytes);
 /* device_ptr: DEVICE memory of at least `bytes` (256-byte aligned); cuda_stream: cudaStream_t. */
 int tdr_bind_workspace(tdr_problem *, void *device_ptr, uint64_t bytes, void *cuda_stream);
-/* D1: ids 0..n-1, generation 0, secondaries followed to extinction. */
+/* Fixed-source run (PAPER.md:103 [section 4]: "a uniform 14 MeV source ... run across a range of source particle counts [and]
+ * temporal tally resolutions"; reading D1): source ids id_offset .. id_offset+n-1, generation 0, secondaries followed to
+ * extinction (or to the census of a time mesh).  HOST scalars; results stay on the device until tdr_read_tallies.
+ * Errors: TDR_ESTATE without a workspace, TDR_ENOMEM if it is too small, TDR_ECAPACITY / TDR_ELOST / TDR_EOVERFLOW from the device. */
 int tdr_run_fixed_source(tdr_problem *, uint64_t n_particles, uint64_t seed);
-/* D2: power iteration with population control; tallies over active generations. */
+/* k-eigenvalue run (PAPER.md:101 [section 4]: "k-eigenvalue simulations, using splitting roulette population control to bound
+ * storage requirements for particle data ... the first ... cycles inactive and the remaining cycles active"; reading D2): power
+ * iteration over n_inactive + n_active generations of about n_particles, k per generation from the track-length estimator,
+ * tallies over the active generations only.  Same error behaviour as above; TDR_ESTATE if the population dies out. */
 int tdr_run_k_eigenvalue(tdr_problem *, uint64_t n_particles, uint32_t n_inactive, uint32_t n_active, uint64_t seed);
 /* D2 in steps, for ONE k-eigenvalue problem shared by several GPUs (one process each; the paper's counterpart is
  * MPI replication over 4 V100s).  Every process holds a contiguous share of the source:
@@ -154,7 +162,9 @@ int tdr_k_population_control(tdr_problem *, uint32_t gen_next, double pr, uint64
 int tdr_k_end(tdr_problem *, uint32_t n_gen, uint32_t n_inactive, const uint64_t *gen_n, const uint64_t *gen_m, const int64_t *gen_p,
               const int64_t *gen_pc, const double *gen_k);
 int tdr_tally_sizes(const tdr_problem *, tdr_sizes *out);
-/* Copies device tallies into the caller's HOST buffers.  TDR_ESTATE before any run. */
+/* The `finalize` side of the method (PAPER.md:65 [section 3]: results leave the device once, after the last event): copies the
+ * int64 fixed-point tallies, leak counts, totals, per-generation sums, per-history records and the last fission bank into the
+ * caller's HOST buffers (NULL = skip; sizes from tdr_tally_sizes).  TDR_ESTATE before any completed run. */
 int tdr_read_tallies(const tdr_problem *, tdr_tallies *out);
 int tdr_read_diagnostics(const tdr_problem *, tdr_diag *out);
 void tdr_free_problem(tdr_problem *);

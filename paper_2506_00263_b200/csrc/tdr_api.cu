@@ -65,7 +65,17 @@ struct tdr_problem {
   // D2 in steps
   u64 k_first = 0, k_nsrc = 0, k_seed = 0, k_last_bank = 0; u32 k_ngen = 0; bool k_keep = false; double k_clock_ms = 0;
   std::vector<cudaEvent_t> ev_pool; size_t ev_used = 0;
+  // stack scheme, device-driven remap loop: a CUDA graph with one WHILE node (built per run), its capture stream, and the
+  // DevRun the graph's kernels read
+  int device_loop = 1;
+  cudaGraph_t sg_graph = nullptr; cudaGraphExec_t sg_exec = nullptr; cudaStream_t sg_capture = nullptr; int sg_per_pass = 0;
+  DevRun *run_dev = nullptr;
 };
+
+static void drop_stack_graph(tdr_problem *p) {
+  if (p->sg_exec) { cudaGraphExecDestroy(p->sg_exec); p->sg_exec = nullptr; }
+  if (p->sg_graph) { cudaGraphDestroy(p->sg_graph); p->sg_graph = nullptr; }
+}
 
 const char *tdr_last_error(void) { return g_err; }
 
@@ -84,6 +94,8 @@ void tdr_free_problem(tdr_problem *p) {
   if (!p) return;
   for (void *d : p->dev_allocs) cudaFree(d);
   for (cudaEvent_t e : p->ev_pool) cudaEventDestroy(e);
+  drop_stack_graph(p);
+  if (p->sg_capture) cudaStreamDestroy(p->sg_capture);
   if (p->h_ctr) cudaFreeHost(p->h_ctr);
   delete p;
 }
@@ -259,6 +271,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "ps_threads") { int n = atoi(value); if (n < 32 || n > PS_THREADS || n % 32) return fail(TDR_EINVAL, "ps_threads: a multiple of 32 in [32,%d]", PS_THREADS); p->ps_threads = n; }
   else if (k == "bank_cap") p->bank_cap_opt = strtoull(value, nullptr, 10);
   else if (k == "arena_links") p->arena_links_opt = strtoull(value, nullptr, 10);
+  else if (k == "device_loop") p->device_loop = atoi(value) != 0;
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -292,6 +305,7 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   u32 *st[EV_COUNT];
   for (int e = 0; e < EV_COUNT; e++) st[e] = c.take<u32>(W);
   u64 *ctr = c.take<u64>(C_COUNT);
+  DevRun *run_dev = c.take<DevRun>(1);
   DevOut o;
   o.flux = c.take<u64>(p->dp.n_bins); o.coll = c.take<u64>(p->dp.n_bins); o.leak = c.take<u64>(6);
   o.totals = c.take<u64>(TDR_T_COUNT); o.PPc = c.take<u64>(2); o.err = c.take<int>(1);
@@ -303,7 +317,7 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   AsyncMem am; async_layout(c, W, sec_cap, p->arena_links_opt, am);
   PsMem pm; pstash_layout(c, W, p->arena_links_opt, pm);
   if (assign) {
-    p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->out = o;
+    p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->run_dev = run_dev; p->out = o;
     p->bank = bank; p->srcbank = src; p->sec = sec; p->sec_time = sec_time; p->sec_w = sec_w; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
     p->hist_cap = hist_cap; p->hist_id = hid; p->hist_nseg = hs; p->hist_ncoll = hc; p->am = am; p->pm = pm;
   }
@@ -358,30 +372,87 @@ static int check_dev_err(tdr_problem *p, int code) {
 
 #define LAUNCH_CHECK() CK(cudaGetLastError())
 
-// ---------------------------------------------------------------------------------- split decomposition (stack scheme)
-template <bool CE>
-static void split_grids(tdr_problem *p, size_t smem, SplitGrids &sg) {
-  sg.g[EV_LOOKUP] = grid_for(p, k_event<CE, EV_LOOKUP>, smem);
-  sg.g[EV_MOVE] = grid_for(p, k_event<CE, EV_MOVE>, smem);
-  sg.g[EV_TALLY] = grid_for(p, k_event<CE, EV_TALLY>, smem);
-  sg.g[EV_COLLIDE] = grid_for(p, k_event<CE, EV_COLLIDE>, smem);
-  sg.g[EV_SURFACE] = grid_for(p, k_event<CE, EV_SURFACE>, smem);
+// ---------------------------------------------------------------------------------- stack scheme: one remap iteration
+// The kernels of remap iteration `it` on stream st: the monolithic step (fused), step + collide (hybrid) or the five event
+// kernels in flow order (split; one kernel per event stack, a kernel whose stack is empty returns at once).  DEV selects
+// where the kernels find their DevRun (TDR_BIND_RUN); `cap_blocks` bounds the grids by the population where it is known.
+struct StackGrids { int step, coll, ev[EV_COUNT]; };
+
+template <bool CE, bool DEV>
+static void stack_grids(tdr_problem *p, size_t smem, StackGrids &g) {
+  memset(&g, 0, sizeof g);
+  if (p->split == 1) {
+    g.ev[EV_LOOKUP] = grid_for(p, k_event<CE, EV_LOOKUP, DEV>, smem); g.ev[EV_MOVE] = grid_for(p, k_event<CE, EV_MOVE, DEV>, smem);
+    g.ev[EV_TALLY] = grid_for(p, k_event<CE, EV_TALLY, DEV>, smem); g.ev[EV_COLLIDE] = grid_for(p, k_event<CE, EV_COLLIDE, DEV>, smem);
+    g.ev[EV_SURFACE] = grid_for(p, k_event<CE, EV_SURFACE, DEV>, smem);
+  } else if (p->split == 2) { g.step = grid_for(p, k_step<CE, true, DEV>, smem); g.coll = grid_for(p, k_collide<CE, DEV>, smem); }
+  else g.step = grid_for(p, k_step<CE, false, DEV>, smem);
 }
 
-// one remap iteration: one kernel per event stack, in flow order; an empty stack costs an empty launch
+template <bool CE, bool DEV>
+static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, size_t smem, const StackGrids &G, u64 it, int cap_blocks) {
+  u64 *ctr = p->ctr;
+  const DevRun *Rp = DEV ? p->run_dev : nullptr;
+  auto cap = [&](int g) { return g < cap_blocks ? g : cap_blocks; };
+  const u32 spl = (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3));
+  if (p->split == 1) {
+    StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
+    K.cnt = ctr + C_STACK0;
+    k_event<CE, EV_LOOKUP, DEV><<<cap(G.ev[EV_LOOKUP]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_SURFACE);
+    k_event<CE, EV_MOVE, DEV><<<cap(G.ev[EV_MOVE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_LOOKUP);
+    k_event<CE, EV_TALLY, DEV><<<cap(G.ev[EV_TALLY]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_MOVE);
+    k_event<CE, EV_COLLIDE, DEV><<<cap(G.ev[EV_COLLIDE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_TALLY);
+    k_event<CE, EV_SURFACE, DEV><<<cap(G.ev[EV_SURFACE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_COLLIDE);
+    return 5;
+  }
+  // fused / hybrid: two index stacks, three rotating counters (in, out, the one to clear)
+  if (DEV) {                                       // the kernels derive the iteration's pointers themselves: bases only
+    if (p->split == 2) {
+      k_step<CE, true, true><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, p->stacks[2], nullptr, nullptr, spl);
+      k_collide<CE, true><<<G.coll, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], ctr, p->stacks[0], reinterpret_cast<u64 *>(p->stacks[1]));
+      return 2;
+    }
+    k_step<CE, false, true><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, nullptr, nullptr, nullptr, spl);
+    return 1;
+  }
+  const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
+  if (p->split == 2) {
+    u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // collide-stack counters
+    k_step<CE, true, DEV><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+                                                          p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, spl);
+    k_collide<CE, DEV><<<cap(G.coll), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], cc, p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
+    return 2;
+  }
+  k_step<CE, false, DEV><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+                                                         p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, spl);
+  return 1;
+}
+
+// the device-driven loop: graph = one WHILE node; body = ONE remap iteration + k_loop_ctl, so the condition (extinct, short
+// enough to drain, error) is tested after every iteration.  Captured once per run on the library's own capture stream.
 template <bool CE>
-static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg, int cap_blocks) {
-  cudaStream_t st = p->stream;
-  StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
-  K.cnt = p->ctr + C_STACK0;
-  auto g = [&](int e) { return sg.g[e] < cap_blocks ? sg.g[e] : cap_blocks; };
-  KTimer t(p, true);
-  k_event<CE, EV_LOOKUP><<<g(EV_LOOKUP), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_SURFACE);
-  k_event<CE, EV_MOVE><<<g(EV_MOVE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_LOOKUP);
-  k_event<CE, EV_TALLY><<<g(EV_TALLY), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_MOVE);
-  k_event<CE, EV_COLLIDE><<<g(EV_COLLIDE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_TALLY);
-  k_event<CE, EV_SURFACE><<<g(EV_SURFACE), 256, smem, st>>>(p->dp, p->out, R, p->soa, K, EV_COLLIDE);
-  LAUNCH_CHECK(); p->diag.kernel_launches += 5;
+static int build_stack_graph(tdr_problem *p, size_t smem) {
+  drop_stack_graph(p);
+  if (!p->sg_capture) CK(cudaStreamCreateWithFlags(&p->sg_capture, cudaStreamNonBlocking));
+  CK(cudaGraphCreate(&p->sg_graph, 0));
+  cudaGraphConditionalHandle h;
+  CK(cudaGraphConditionalHandleCreate(&h, p->sg_graph, 1, cudaGraphCondAssignDefault));
+  cudaGraphNodeParams np = { cudaGraphNodeTypeConditional }; np.conditional.handle = h; np.conditional.type = cudaGraphCondTypeWhile; np.conditional.size = 1;
+  cudaGraphNode_t node;
+  CK(cudaGraphAddNode(&node, p->sg_graph, nullptr, 0, &np));
+  cudaGraph_t body = np.conditional.phGraph_out[0];
+  StackGrids G; stack_grids<CE, true>(p, smem, G);
+  DevRun none; memset(&none, 0, sizeof none);
+  CK(cudaStreamBeginCaptureToGraph(p->sg_capture, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
+  const int per_pass = remap_iteration<CE, true>(p, none, p->sg_capture, smem, G, 0, 1 << 30);
+  LoopCtl c; c.ctr = p->ctr; c.R = p->run_dev; c.split = p->split == 1; c.drain_below = (u64)p->drain_below;
+  k_loop_ctl<<<1, 32, 0, p->sg_capture>>>(c, h);
+  cudaGraph_t captured = nullptr;
+  cudaError_t e = cudaStreamEndCapture(p->sg_capture, &captured);
+  if (e != cudaSuccess) { drop_stack_graph(p); return fail(TDR_ECUDA, "capture of the remap loop failed: %s", cudaGetErrorString(e)); }
+  e = cudaGraphInstantiate(&p->sg_exec, p->sg_graph, 0);
+  if (e != cudaSuccess) { drop_stack_graph(p); return fail(TDR_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e)); }
+  p->sg_per_pass = per_pass;
   return 0;
 }
 
@@ -406,62 +477,57 @@ static int run_stack(tdr_problem *p, DevRun R) {
     return 0;
   };
   int rc;
+  const bool split = p->split == 1, dev = p->device_loop != 0;
+  // the live stack between iterations: stacks[it & 1] with counter it % 3 (fused, hybrid), the LOOKUP stack (split)
+  auto live_stack = [&](u64 it) { return split ? p->stacks[EV_LOOKUP] : p->stacks[it & 1]; };
+  auto live_count = [&](u64 it) { return ctr + C_STACK0 + (split ? (u64)EV_LOOKUP : it % 3); };
   u64 n0 = R.src_total < W ? R.src_total : W;
-  // fused: two index stacks, three rotating counters (in, out, the one to clear); split: one stack per event
-  u64 it = 0;
-  const bool split = p->split == 1, hybrid = p->split == 2;
-  if (!split) { if ((rc = source(p->stacks[0], ctr + C_STACK0, 0, n0))) return rc; }
-  else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, 0, n0))) return rc;
+  u64 it = 0, passes_seen = 0;
+  if ((rc = source(live_stack(0), live_count(0), 0, n0))) return rc;
   u64 n_in = n0;
-  const int g_step = split ? 0 : hybrid ? grid_for(p, k_step<CE, true>, smem) : grid_for(p, k_step<CE, false>, smem);
-  const int g_coll = hybrid ? grid_for(p, k_collide<CE>, smem) : 0;
-  SplitGrids sg; if (split) split_grids<CE>(p, smem, sg);
+  StackGrids G;
+  if (dev) { if (!p->sg_exec && (rc = build_stack_graph<CE>(p, smem))) return rc; }
+  else stack_grids<CE, false>(p, smem, G);
   for (;;) {
     R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
-    // the out count never exceeds the in count (dead lanes are reborn in place), so n_in bounds every launch of
-    // this batch: launch `batch` remap iterations back to back and read the counters once
-    const int batch = n_in * 4 > W ? 1 : p->sync_every;
-    u64 blocks64 = (n_in + 255) / 256; int cap_blocks = blocks64 > (1u << 30) ? (1 << 30) : (int)blocks64;
-    if (cap_blocks < 1) cap_blocks = 1;
-    {
-    KTimer tb(p, !split, batch * (hybrid ? 2 : 1));     // one event pair per batch: the launches run back to back
-    for (int b = 0; b < batch; b++) {
-      if (!split) {
-        const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
-        u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // hybrid: collide-stack counters
-        const int g1 = g_step < cap_blocks ? g_step : cap_blocks;
-        if (hybrid) {
-          k_step<CE, true><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                  p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3)));
-          k_collide<CE><<<g_coll < cap_blocks ? g_coll : cap_blocks, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[2], cc,
-                                                                                     p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
-          p->diag.kernel_launches++;
-        } else
-          k_step<CE, false><<<g1, 256, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                   p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3)));
-        LAUNCH_CHECK(); p->diag.kernel_launches++;
-      } else if ((rc = split_iteration<CE>(p, R, smem, sg, cap_blocks))) return rc;
-      it++; p->diag.iterations++;
-    }
+    if (dev) {
+      // one graph launch runs remap iterations until the population is extinct (or short enough to drain, or an error is
+      // flagged); the host comes back for the tail drain, for a refill of an empty window, or to finish
+      CK(cudaMemcpyAsync(p->run_dev, &R, sizeof R, cudaMemcpyHostToDevice, st));      // (pageable source: staged before the call returns)
+      { KTimer tb(p, true, 0); CK(cudaGraphLaunch(p->sg_exec, st)); }
+    } else {
+      // the out count never exceeds the in count (dead lanes are reborn in place), so n_in bounds every launch of
+      // this batch: launch `batch` remap iterations back to back and read the counters once
+      const int batch = n_in * 4 > W ? 1 : p->sync_every;
+      u64 blocks64 = (n_in + 255) / 256; int cap_blocks = blocks64 > (1u << 30) ? (1 << 30) : (int)blocks64;
+      if (cap_blocks < 1) cap_blocks = 1;
+      KTimer tb(p, true, 0);                              // one event pair per batch: the launches run back to back
+      for (int b = 0; b < batch; b++) {
+        const int nk = remap_iteration<CE, false>(p, R, st, smem, G, it, cap_blocks);
+        LAUNCH_CHECK(); p->diag.kernel_launches += nk; p->diag.step_launches += p->time_kernels ? nk : 0;
+        it++; p->diag.iterations++;
+      }
     }
     CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
     CK(cudaStreamSynchronize(st));
+    if (dev) {
+      const u64 np = h[C_PENDING] - passes_seen; passes_seen = h[C_PENDING];
+      it = h[C_PENDING]; p->diag.iterations += np;
+      p->diag.kernel_launches += np * (p->sg_per_pass + 1); p->diag.step_launches += p->time_kernels ? np * (p->sg_per_pass + 1) : 0;
+    }
     if ((rc = check_dev_err(p, (int)h[C_COUNT - 1]))) return rc;
-    const u64 alive = split ? h[C_STACK0 + EV_LOOKUP] : h[C_STACK0 + it % 3];
+    const u64 alive = h[C_STACK0 + (split ? (u64)EV_LOOKUP : it % 3)];
     n_in = alive;
     h_sec_tail = h[C_SEC_TAIL];
     h_src_next = h[C_SRC_NEXT] < R.src_total ? h[C_SRC_NEXT] : R.src_total;
     h_sec_head = h[C_SEC_HEAD] < R.sec_limit ? h[C_SEC_HEAD] : R.sec_limit;          // claims past the limit got nothing
+    if (dev) h_sec_head = h[C_SEC_HEAD];                                              // (k_loop_ctl has already given them back)
     const u64 pend = h_sec_tail - h_sec_head, rem = R.src_total - h_src_next;
     if (R.kmode && rem == 0 && alive > 0 && alive <= (u64)p->drain_below) {
       // tail drain: the few particles left are followed to their death in ONE launch (k_drain).  Also under the five-event
       // decomposition: after a whole iteration every survivor waits on the LOOKUP stack, i.e. at the start of a segment.
       const int blocks = (int)((alive + 63) / 64);
-      {
-        KTimer td(p, true);
-        if (split) k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP);
-        else k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, p->stacks[it & 1], ctr + C_STACK0 + it % 3);
-      }
+      { KTimer td(p, true); k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, live_stack(it), live_count(it)); }
       LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.iterations++;
       CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
       CK(cudaStreamSynchronize(st));
@@ -472,10 +538,9 @@ static int run_stack(tdr_problem *p, DevRun R) {
       if (pend + rem == 0) break;
       u64 n = pend + rem < W ? pend + rem : W, n_sec = pend < n ? pend : n;
       R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
-      if (!split) { if ((rc = source(p->stacks[it & 1], ctr + C_STACK0 + it % 3, n_sec, n))) return rc; }
-      else if ((rc = source(p->stacks[EV_LOOKUP], ctr + C_STACK0 + EV_LOOKUP, n_sec, n))) return rc;
+      if ((rc = source(live_stack(it), live_count(it), n_sec, n))) return rc;
       n_in = n;
-    } else if (h[C_SEC_HEAD] != h_sec_head) {
+    } else if (!dev && h[C_SEC_HEAD] != h_sec_head) {
       h[33] = h_sec_head;                                   // clamp the overshoot of the claim cursor (the limit grows later)
       CK(cudaMemcpyAsync(ctr + C_SEC_HEAD, h + 33, 8, cudaMemcpyHostToDevice, st));
       CK(cudaStreamSynchronize(st));
@@ -644,6 +709,7 @@ static int begin_run(tdr_problem *p, u64 n) {
   p->ran = false; p->gen_n.clear(); p->gen_m.clear(); p->gen_p.clear(); p->gen_pc.clear(); p->gen_k.clear();
   p->k_mean = p->k_std = 0; p->n_hist = p->n_bank = 0;
   memset(&p->diag, 0, sizeof p->diag); p->ev_used = 0;
+  drop_stack_graph(p);                         // the graph's kernel arguments are this run's pointers and options
   return 0;
 }
 

@@ -359,7 +359,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O
     if (starved) { starved = false; backoff = 250; if (w.lane == 0) atomicAdd(R.starved, ~0ull); }
     if ((n_iter & 1023u) == 1023u) {                              // hard watchdog for a warp that stays busy
       int ex = 0;
-      if (w.lane == 0 && global_ns() - t_start > 40 * deadline_ns) {
+      if (w.lane == 0 && global_ns() - t_start > 4 * deadline_ns) {
         ex = 1; atomicExch(O.err, TDR_ELOST);
         A.actr[AC_DBG] = w.gw; A.actr[AC_DBG + 1] = (u64)s.cnt(l); A.actr[AC_DBG + 2] = (u64)s.ev(l); A.actr[AC_DBG + 3] = (u64)s.nfull();
         A.actr[AC_DBG + 4] = (u64)s.nfree(); A.actr[AC_DBG + 5] = n_iter; A.actr[AC_DBG + 6] = n_events; A.actr[AC_DBG + 7] = (u64)delta;

@@ -31,8 +31,8 @@ enum { CE_MOVE = 0, CE_COLLIDE = 1, CE_BIRTH = 2, CE_IDLE = 3, CE_EXIT = 4 };
 struct CsCtl {                              // CTA-wide scheduler state in shared memory
   u32 tail[3], head[3];                     // monotonically increasing counters; ring index = counter & mask
   u32 ev, base, n;                          // the round descriptor
-  u32 primary_done, open_total, reaping, gwork_hint, starved, backoff;
-  unsigned long long t_idle, last_out;
+  u32 primary_done, open_total, reaping, gwork_hint, starved, backoff, rounds;
+  unsigned long long t_idle, last_out, t_start;
 };
 
 template <bool CE>
@@ -138,7 +138,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
     for (int r = 0; r < 3; r++) { ctl.tail[r] = 0; ctl.head[r] = 0; }
     ctl.tail[CE_BIRTH] = (u32)NS;
     ctl.primary_done = 0; ctl.open_total = 0; ctl.reaping = 0; ctl.gwork_hint = 0; ctl.starved = 0; ctl.backoff = 250;
-    ctl.t_idle = 0; ctl.last_out = ~0ull;
+    ctl.t_idle = 0; ctl.last_out = ~0ull; ctl.rounds = 0; ctl.t_start = global_ns();
   }
   acc_init(&acc);                             // (ends with a barrier)
   PsWarp w;
@@ -151,13 +151,16 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
     if (threadIdx.x == 0) {
       const u32 cM = ctl.tail[CE_MOVE] - ctl.head[CE_MOVE], cC = ctl.tail[CE_COLLIDE] - ctl.head[CE_COLLIDE], cB = ctl.tail[CE_BIRTH] - ctl.head[CE_BIRTH];
       bool can_birth = !ctl.primary_done;
-      if (!can_birth && !R.kmode) {
-        if (ctl.open_total > 0) can_birth = true;
-        else if (cB >= 32 && (cM + cC < cap)) {                   // worth a look at the global queues (an L2 round trip)
-          ctl.gwork_hint = (u32)ld_vol(&A.ctr[PC_GWORK]);
-          can_birth = ctl.gwork_hint > 0;
-        }
+      if (!R.kmode) {
+        // a look at the global queues (one L2 round trip) before any round that could be a birth round: full links are taken
+        // BEFORE new source particles (depth first), so the links in flight stay bounded by what the resident particles
+        // produce however long the source is; once the source is exhausted, the look decides whether births are possible
+        const bool birth_in_reach = can_birth ? (cB >= cap || (cB > cM && cB > cC)) : (ctl.open_total == 0 && cB >= 32 && cM + cC < cap);
+        if (birth_in_reach) ctl.gwork_hint = (u32)ld_vol(&A.ctr[PC_GWORK]);
+        if (!can_birth) can_birth = ctl.open_total > 0 || (cB >= 32 && ctl.gwork_hint > 0);
       }
+      // hard watchdog (a scheduler that stopped making progress must end in an error code, not in a hung device)
+      if ((++ctl.rounds & 4095u) == 0 && !ctl.reaping && global_ns() - ctl.t_start > 4 * deadline_ns) { atomicExch(O.err, TDR_ELOST); ctl.reaping = 1; }
       u32 ev;
       if (ctl.reaping) ev = cB > 0 ? CE_BIRTH : CE_EXIT;
       else if (cC >= cap) ev = CE_COLLIDE;
@@ -197,7 +200,16 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
     }
     const u32 my = wid * 32;
     const u32 n = ctl.n > my ? min(32u, ctl.n - my) : 0u;
-    if (n == 0) continue;
+    if (n == 0) {
+      // a BIRTH round that brought this warp no free slot while it sits on secondaries and the source is exhausted: publish
+      // them, so that whichever warp does get slots can take them (otherwise the round could repeat unchanged for ever)
+      if (ev == CE_BIRTH && !R.kmode && w.open_count > 0 && ctl.primary_done) {
+        ps_open_deposit(w);
+        if (lane == 0) atomicAdd(&ctl.open_total, 0u - open_pub);
+        open_pub = 0;
+      }
+      continue;
+    }
     const bool valid = lane < n;
     const u32 slot = valid ? (u32)pl.ring[ev][(ctl.base + my + lane) & pl.mask] : 0u;
 
@@ -212,28 +224,10 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOu
       }
       if (ctl.reaping) continue;
       Part p; bool born = false;
-      if (!R.kmode) {
-        const u32 t = min(n, w.open_count);                       // (1) this warp's own secondaries, newest first
-        if (t) {
-          if (lane < t) { const tdr_site s = load_site_cg(&A.links[w.open_id].s[w.open_count - t + lane]); birth_site<CE>(P, mg, R, &acc, p, s); born = true; }
-          w.open_count -= t;
-        } else if (n == 32 && ctl.primary_done && ctl.gwork_hint > 0) {   // (2) fetch: a whole link
-          u32 g = NOLINK;
-          if (lane == 0) g = q_pop(A.links, A.q_work, w.gw, 2);
-          g = __shfl_sync(FULL, g, 0);
-          if (g != NOLINK) {
-            const u32 c = __ldcg(&A.links[g].count);
-            if (lane < c) { const tdr_site s = load_site_cg(&A.links[g].s[lane]); birth_site<CE>(P, mg, R, &acc, p, s); born = true; }
-            __syncwarp();
-            if (lane == 0) {
-              atomicAdd(&A.ctr[PC_GWORK], ~0ull);
-              *(volatile u32 *)&A.links[g].next = NOLINK;
-              __threadfence();
-              q_deposit(A.links, A.q_empty, w.gw % AQ, ((u64)g << 32) | g);
-            }
-            w.n_fetch++;
-          }
-        }
+      if (!R.kmode) {                                             // (1), (2): secondaries first (the warp's open link, then the global queues)
+        u32 hint = ctl.gwork_hint;
+        born = ps_birth_from_links<CE>(w, P, mg, R, &acc, p, n, hint);
+        if (hint == 0 && lane == 0) ctl.gwork_hint = 0;           // the hint was stale: no further attempt before it is read again
       }
       const u32 m = __ballot_sync(FULL, valid && !born);          // (3) the primary source: one atomic per warp
       if (m && !*(volatile u32 *)&ctl.primary_done) {

@@ -148,6 +148,44 @@ __device__ TDR_COLD void ps_push_secondaries(PsWarp &w, const DevRun &R, BlockAc
   __syncwarp();
 }
 
+// SOURCE event of a fixed-source run: secondaries BEFORE new source particles (depth first), so the links in flight stay
+// bounded by what the resident particles produce however long the source is.  Lanes [0, n) of the warp hold a free slot.
+// (1) the warp's open link, newest record first; (2) when it runs dry and full links wait in the global queues, one of
+// them becomes the open link (the fetch of PAPER.md:87, 95: claimed whole, so nobody waits on a writer) and serves the
+// rest.  Returns true for a lane that was born from a site; gwork_hint is cleared when the queues in reach were empty.
+template <bool CE>
+__device__ __forceinline__ bool ps_birth_from_links(PsWarp &w, const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
+                                                    u32 n, u32 &gwork_hint) {
+  bool born = false; u32 served = 0;
+  for (int round = 0; round < 2; round++) {
+    const u32 t = min(n - served, w.open_count);
+    if (t) {
+      if (w.lane >= served && w.lane < served + t) {
+        const tdr_site s = load_site_cg(&w.A.links[w.open_id].s[w.open_count - t + (w.lane - served)]);
+        birth_site<CE>(P, mg, R, acc, p, s); born = true;
+      }
+      w.open_count -= t; served += t;
+    }
+    if (served == n || round == 1 || gwork_hint == 0) break;
+    u32 g = NOLINK;                                  // the open link is empty here
+    if (w.lane == 0) g = q_pop(w.A.links, w.A.q_work, w.gw, 4);
+    g = __shfl_sync(FULL, g, 0);
+    if (g == NOLINK) { gwork_hint = 0; break; }
+    const u32 c = __ldcg(&w.A.links[g].count);
+    if (w.lane == 0) {
+      atomicAdd(&w.A.ctr[PC_GWORK], ~0ull);
+      if (w.open_id != NOLINK) {                     // hand the old (empty) open link back
+        *(volatile u32 *)&w.A.links[w.open_id].next = NOLINK;
+        __threadfence();
+        q_deposit(w.A.links, w.A.q_empty, w.gw % AQ, ((u64)w.open_id << 32) | w.open_id);
+      }
+    }
+    __syncwarp();
+    w.open_id = g; w.open_count = c; w.n_fetch++;
+  }
+  return born;
+}
+
 #ifndef PS_THREADS
 #define PS_THREADS 256
 #endif
@@ -179,8 +217,14 @@ __global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P, DevOu
   u32 n_iter = 0, backoff = 250, gwork_hint = 0, starved_hint = 0;
   u32 ev_cnt[3] = { 0, 0, 0 }, ln_cnt[3] = { 0, 0, 0 };
   u64 t_idle = 0, last_out = ~0ull;
+  const u64 t_start = global_ns();
   enum { E_MOVE = 0, E_COLLIDE = 1, E_BIRTH = 2 };
   for (;;) {
+    if ((n_iter & 4095u) == 4095u) {           // hard watchdog: a warp that stays busy for ever ends in an error code, not in a hung device
+      int ex = 0;
+      if (lane == 0 && global_ns() - t_start > 4 * deadline_ns) { ex = 1; atomicExch(O.err, TDR_ELOST); }
+      if (__shfl_sync(FULL, ex, 0)) break;
+    }
     // periodic housekeeping of a busy warp: publish the outstanding delta; fixed source: look at the global queues
     if ((++n_iter & 31u) == 0) {
       if (delta != 0) { if (lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
@@ -192,8 +236,7 @@ __global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P, DevOu
         if (starved_hint > 0 && w.open_count > 0 && mq.count + cq.count >= 32) ps_open_deposit(w);
       }
     }
-    // a fetch takes a whole global link, so it needs a whole warp of free slots
-    const bool can_birth = !primary_done || (!R.kmode && (w.open_count > 0 || (gwork_hint > 0 && bq.count >= 32)));
+    const bool can_birth = !primary_done || (!R.kmode && (w.open_count > 0 || gwork_hint > 0));
     int ev;
     if (cq.count >= 32) ev = E_COLLIDE;
     else if (mq.count >= 32) ev = E_MOVE;
@@ -225,28 +268,9 @@ __global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P, DevOu
       const bool want = lane < n;
       const u32 slot = bq.pop(n, lane);
       Part p; bool born = false;
-      if (!R.kmode) {
-        const u32 t = min(n, w.open_count);                       // (1) this warp's own secondaries, newest first
-        if (t) {
-          if (lane < t) { const tdr_site s = load_site_cg(&A.links[w.open_id].s[w.open_count - t + lane]); birth_site<CE>(P, mg, R, &acc, p, s); born = true; }
-          w.open_count -= t;
-        } else if (n == 32 && gwork_hint > 0) {                   // (2) fetch: a whole link from the global queues
-          u32 g = NOLINK;
-          if (lane == 0) g = q_pop(A.links, A.q_work, w.gw, 2);
-          g = __shfl_sync(FULL, g, 0);
-          if (g != NOLINK) {
-            const u32 c = __ldcg(&A.links[g].count);
-            if (lane < c) { const tdr_site s = load_site_cg(&A.links[g].s[lane]); birth_site<CE>(P, mg, R, &acc, p, s); born = true; }
-            __syncwarp();
-            if (lane == 0) {
-              atomicAdd(&A.ctr[PC_GWORK], ~0ull);
-              *(volatile u32 *)&A.links[g].next = NOLINK;
-              __threadfence();
-              q_deposit(A.links, A.q_empty, w.gw % AQ, ((u64)g << 32) | g);
-            }
-            w.n_fetch++;
-          } else gwork_hint = 0;
-        }
+      if (!R.kmode) {                                             // (1), (2): secondaries first
+        if (w.open_count < n) { u32 g = 0; if (lane == 0) g = (u32)ld_vol(&A.ctr[PC_GWORK]); gwork_hint = __shfl_sync(FULL, g, 0); }
+        born = ps_birth_from_links<CE>(w, P, mg, R, &acc, p, n, gwork_hint);
       }
       const u32 m = __ballot_sync(FULL, want && !born);           // (3) the primary source: one atomic per warp
       if (m && !primary_done) {

@@ -8,10 +8,11 @@
 
 struct StackSet { u32 *s[EV_COUNT]; u64 *cnt; };      // cnt[e] = device counter of stack e
 
-template <bool CE, int EV>
-__global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun R, Soa S, StackSet K, int zero_ev) {
+template <bool CE, int EV, bool DEV>
+__global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, StackSet K, int zero_ev) {
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
+  TDR_BIND_RUN(DEV, Rv, Rp)
   const double *mg = stage_mg(P, smem);
   const TallyPriv tp = stage_priv(P, smem);
   acc_init(&acc);
@@ -43,11 +44,19 @@ __global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun R, So
 
 // hybrid scheme, second kernel of a remap iteration: the COLLIDE event on the collide stack; survivors (and lanes
 // reborn by make_work) join the step stack the preceding k_step<CE, true> launch was pushing to.
-template <bool CE>
-__global__ void __launch_bounds__(256) k_collide(DevProb P, DevOut O, DevRun R, Soa S, const u32 *cstack, const u64 *ccount,
+template <bool CE, bool DEV>
+__global__ void __launch_bounds__(256) k_collide(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, const u32 *cstack, const u64 *ccount,
                                                  u32 *stack_out, u64 *count_out) {
+  if (DEV) {                                       // bases in, this iteration's pointers out (see k_step)
+    u64 *ctr = const_cast<u64 *>(ccount);
+    const u64 it = ctr[C_PENDING];
+    ccount = ctr + C_STACK0 + 3 + (it & 1);
+    u32 *s0 = stack_out, *s1 = reinterpret_cast<u32 *>(count_out);
+    stack_out = (it & 1) ? s0 : s1; count_out = ctr + C_STACK0 + (it + 1) % 3;
+  }
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
+  TDR_BIND_RUN(DEV, Rv, Rp)
   const double *mg = stage_mg(P, smem);
   const TallyPriv tp = stage_priv(P, smem);
   acc_init(&acc);
@@ -66,9 +75,3 @@ __global__ void __launch_bounds__(256) k_collide(DevProb P, DevOut O, DevRun R, 
   acc_flush(&acc, O, accP, accPc);
 }
 
-struct SplitGrids { int g[EV_COUNT]; };
-
-// host side -----------------------------------------------------------------------------------------------
-struct tdr_problem;
-template <bool CE> static void split_grids(tdr_problem *p, size_t smem, SplitGrids &sg);
-template <bool CE> static int split_iteration(tdr_problem *p, DevRun &R, size_t smem, const SplitGrids &sg, int cap_blocks);

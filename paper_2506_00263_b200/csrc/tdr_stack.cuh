@@ -122,19 +122,42 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
   acc_flush(&acc, O, 0, 0);
 }
 
+// ---------------------------------------------------------------------------------- where a remap kernel finds its DevRun
+// DEV = false: by value, the host drives the remap loop and reads the counters back between batches.  DEV = true: from
+// device memory, copied to shared memory at kernel start — the remap loop then runs as a CUDA-graph WHILE node whose last
+// kernel (k_loop_ctl) updates the claimable range of the secondary ring and decides whether another pass is needed, so the
+// host is out of the loop ("fixed costs": the launch and read-back latency of every remap iteration).
+#define TDR_BIND_RUN(DEV, Rv, Rp)                                                                                               \
+  __shared__ DevRun Rs_;                                                                                                        \
+  if (DEV) { for (u32 i_ = threadIdx.x; i_ < (u32)(sizeof(DevRun) / 8); i_ += blockDim.x) ((u64 *)&Rs_)[i_] = ((const u64 *)(Rp))[i_]; } \
+  const DevRun &R = DEV ? Rs_ : Rv;        /* visible after the barrier that ends acc_init */
+
 // ---------------------------------------------------------------------------------- fused STEP (monolithic scheme)
 // HYBRID: a particle that collides is not processed here; it is pushed onto the collide stack (cstack) and the
 // collision runs as its own event in k_collide, where every lane of a warp takes the same path.
-template <bool CE, bool HYBRID>
-__global__ void __launch_bounds__(256) k_step(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in,
+// The step stacks alternate and their counters rotate by three (in, out, the one to clear) with the remap iteration `it`.
+// The host-driven loop passes the pointers of its iteration; the device-driven loop passes the bases (stack_in = stack 0,
+// stack_out = stack 1, count_in = the counter block `ctr`) and every kernel derives its own from the iteration counter that
+// k_loop_ctl keeps in ctr[C_PENDING] — so the WHILE body is ONE iteration and the loop condition is tested after each.
+template <bool CE, bool HYBRID, bool DEV>
+__global__ void __launch_bounds__(256, 2) k_step(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, const u32 *stack_in, const u64 *count_in,
                                               u32 *stack_out, u64 *count_out, u64 *count_zero,
                                               u32 *cstack, u64 *ccount, u64 *ccount_zero, u32 seg_per_launch) {
+  if (DEV) {
+    u64 *ctr = const_cast<u64 *>(count_in);
+    const u64 it = ctr[C_PENDING];
+    u32 *s0 = const_cast<u32 *>(stack_in), *s1 = stack_out;
+    stack_in = (it & 1) ? s1 : s0; stack_out = (it & 1) ? s0 : s1;
+    count_in = ctr + C_STACK0 + it % 3; count_out = ctr + C_STACK0 + (it + 1) % 3; count_zero = ctr + C_STACK0 + (it + 2) % 3;
+    if (HYBRID) { ccount = ctr + C_STACK0 + 3 + (it & 1); ccount_zero = ctr + C_STACK0 + 3 + ((it + 1) & 1); }
+  }
   if (blockIdx.x == 0 && threadIdx.x == 0) {       // the stacks the previous launches drained (rotating counters)
     *count_zero = 0;
     if (HYBRID) *ccount_zero = 0;
   }
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
+  TDR_BIND_RUN(DEV, Rv, Rp)
   const double *mg = stage_mg(P, smem);
   const TallyPriv tp = stage_priv(P, smem);
   acc_init(&acc);
@@ -214,6 +237,27 @@ __global__ void __launch_bounds__(256) k_drain(DevProb P, DevOut O, DevRun R, So
   }
   acc_flush(&acc, O, accP, accPc);
   priv_flush(tp, O);
+}
+
+// ---------------------------------------------------------------------------------- device-driven remap loop: the WHILE condition
+// Last kernel of a pass of the graph's body (one thread).  It does what the host does between two batches of the host-driven
+// loop: every kernel of the pass has completed, so every secondary below the ring's tail is whole and claimable; claims past
+// the old limit got nothing and are given back.  Another pass follows while particles are alive, no error is flagged and the
+// k-mode tail has not become short enough for k_drain.
+struct LoopCtl { u64 *ctr; DevRun *R; int split; u64 drain_below; };
+__global__ void k_loop_ctl(LoopCtl c, cudaGraphConditionalHandle h) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  u64 *ctr = c.ctr; DevRun *R = c.R;
+  const u64 it = ctr[C_PENDING] + 1;               // iterations made (the stack scheme has no other use for this counter)
+  ctr[C_PENDING] = it;
+  const u64 alive = ctr[C_STACK0 + (c.split ? (u64)EV_LOOKUP : it % 3)];
+  const int err = *(const int *)(ctr + (C_COUNT - 1));
+  u64 head = ctr[C_SEC_HEAD];
+  if (head > R->sec_limit) { head = R->sec_limit; ctr[C_SEC_HEAD] = head; }
+  R->sec_limit = ctr[C_SEC_TAIL]; R->sec_head0 = head;
+  const bool exhausted = ctr[C_SRC_NEXT] >= R->src_total;
+  const bool drain = R->kmode && exhausted && alive <= c.drain_below;
+  cudaGraphSetConditional(h, (alive > 0 && err == 0 && !drain) ? 1u : 0u);
 }
 
 // ---------------------------------------------------------------------------------- A9 population control (D2)

@@ -134,14 +134,25 @@ def test_async_spill_and_fetch_through_the_global_queues(decomp):
 
 
 # ------------------------------------------------------------------ round 2: holes named by the round-1 review
-@pytest.mark.parametrize("decomp", ["fused", "hybrid"])
-def test_stack_remap_loop_runs_to_extinction_without_the_tail_drain(decomp):
+@pytest.mark.parametrize("device_loop", [1, 0])
+@pytest.mark.parametrize("decomp", ["fused", "hybrid", "split"])
+def test_stack_remap_loop_runs_to_extinction_without_the_tail_drain(decomp, device_loop):
     """drain_below = 0: the k-mode stack scheme never hands the tail to k_drain, so the remap loop itself (rotating
-    counters, the collide-stack hand-off of the hybrid, many iterations of a dwindling population) runs to the last particle."""
+    counters, the collide-stack hand-off of the hybrid, many iterations of a dwindling population) runs to the last particle
+    — as a CUDA-graph WHILE node on the device (device_loop = 1, the default) and in host-driven batches (0)."""
     for p in (W.cfg1(n=30011, n_inactive=1, n_active=2), W.cfg4(n=20011, n_inactive=1, n_active=1)):
-        o, g, d = run_both(p, scheme="stack", decomposition=decomp, drain_below=0)
-        assert_same(o, g, f"{p.name}/stack/{decomp}/drain_below=0")
-        assert d["iterations"] > 50, d
+        o, g, d = run_both(p, scheme="stack", decomposition=decomp, drain_below=0, device_loop=device_loop)
+        assert_same(o, g, f"{p.name}/stack/{decomp}/drain_below=0/device_loop={device_loop}")
+        assert d["iterations"] > 30, d
+
+
+@pytest.mark.parametrize("decomp", ["fused", "hybrid", "split"])
+def test_stack_host_driven_loop_matches_too(decomp):
+    """device_loop = 0 (the round-1 driver: batches of sync_every launches, counters read back by the host) on a fixed source
+    with secondaries, a small window that must be refilled, and a k-eigenvalue run with the tail drain."""
+    for p, kw in ((W.cfg3(n=5003, n_ebins=100), dict(window=1024)), (W.cfg3(n=20011, n_ebins=1), {}), (W.cfg1(n=30011, n_inactive=1, n_active=1), {})):
+        o, g, d = run_both(p, scheme="stack", decomposition=decomp, device_loop=0, **kw)
+        assert_same(o, g, f"{p.name}/stack/{decomp}/device_loop=0")
 
 
 @pytest.mark.parametrize("scheme,decomp", SCHEMES)
