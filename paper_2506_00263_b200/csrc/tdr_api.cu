@@ -378,18 +378,18 @@ static int check_dev_err(tdr_problem *p, int code) {
 // where the kernels find their DevRun (TDR_BIND_RUN); `cap_blocks` bounds the grids by the population where it is known.
 struct StackGrids { int step, coll, ev[EV_COUNT]; };
 
-template <bool CE, bool DEV>
+template <bool CE, bool DEV, bool EXT>
 static void stack_grids(tdr_problem *p, size_t smem, StackGrids &g) {
   memset(&g, 0, sizeof g);
   if (p->split == 1) {
-    g.ev[EV_LOOKUP] = grid_for(p, k_event<CE, EV_LOOKUP, DEV>, smem); g.ev[EV_MOVE] = grid_for(p, k_event<CE, EV_MOVE, DEV>, smem);
-    g.ev[EV_TALLY] = grid_for(p, k_event<CE, EV_TALLY, DEV>, smem); g.ev[EV_COLLIDE] = grid_for(p, k_event<CE, EV_COLLIDE, DEV>, smem);
-    g.ev[EV_SURFACE] = grid_for(p, k_event<CE, EV_SURFACE, DEV>, smem);
-  } else if (p->split == 2) { g.step = grid_for(p, k_step<CE, true, DEV>, smem); g.coll = grid_for(p, k_collide<CE, DEV>, smem); }
-  else g.step = grid_for(p, k_step<CE, false, DEV>, smem);
+    g.ev[EV_LOOKUP] = grid_for(p, k_event<CE, EV_LOOKUP, DEV, EXT>, smem); g.ev[EV_MOVE] = grid_for(p, k_event<CE, EV_MOVE, DEV, EXT>, smem);
+    g.ev[EV_TALLY] = grid_for(p, k_event<CE, EV_TALLY, DEV, EXT>, smem); g.ev[EV_COLLIDE] = grid_for(p, k_event<CE, EV_COLLIDE, DEV, EXT>, smem);
+    g.ev[EV_SURFACE] = grid_for(p, k_event<CE, EV_SURFACE, DEV, EXT>, smem);
+  } else if (p->split == 2) { g.step = grid_for(p, k_step<CE, true, DEV, EXT>, smem); g.coll = grid_for(p, k_collide<CE, DEV, EXT>, smem); }
+  else g.step = grid_for(p, k_step<CE, false, DEV, EXT>, smem);
 }
 
-template <bool CE, bool DEV>
+template <bool CE, bool DEV, bool EXT>
 static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, size_t smem, const StackGrids &G, u64 it, int cap_blocks) {
   u64 *ctr = p->ctr;
   const DevRun *Rp = DEV ? p->run_dev : nullptr;
@@ -398,39 +398,39 @@ static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, siz
   if (p->split == 1) {
     StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
     K.cnt = ctr + C_STACK0;
-    k_event<CE, EV_LOOKUP, DEV><<<cap(G.ev[EV_LOOKUP]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_SURFACE);
-    k_event<CE, EV_MOVE, DEV><<<cap(G.ev[EV_MOVE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_LOOKUP);
-    k_event<CE, EV_TALLY, DEV><<<cap(G.ev[EV_TALLY]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_MOVE);
-    k_event<CE, EV_COLLIDE, DEV><<<cap(G.ev[EV_COLLIDE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_TALLY);
-    k_event<CE, EV_SURFACE, DEV><<<cap(G.ev[EV_SURFACE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_COLLIDE);
+    k_event<CE, EV_LOOKUP, DEV, EXT><<<cap(G.ev[EV_LOOKUP]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_SURFACE);
+    k_event<CE, EV_MOVE, DEV, EXT><<<cap(G.ev[EV_MOVE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_LOOKUP);
+    k_event<CE, EV_TALLY, DEV, EXT><<<cap(G.ev[EV_TALLY]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_MOVE);
+    k_event<CE, EV_COLLIDE, DEV, EXT><<<cap(G.ev[EV_COLLIDE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_TALLY);
+    k_event<CE, EV_SURFACE, DEV, EXT><<<cap(G.ev[EV_SURFACE]), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, K, EV_COLLIDE);
     return 5;
   }
   // fused / hybrid: two index stacks, three rotating counters (in, out, the one to clear)
   if (DEV) {                                       // the kernels derive the iteration's pointers themselves: bases only
     if (p->split == 2) {
-      k_step<CE, true, true><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, p->stacks[2], nullptr, nullptr, spl);
-      k_collide<CE, true><<<G.coll, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], ctr, p->stacks[0], reinterpret_cast<u64 *>(p->stacks[1]));
+      k_step<CE, true, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, p->stacks[2], nullptr, nullptr, spl);
+      k_collide<CE, true, EXT><<<G.coll, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], ctr, p->stacks[0], reinterpret_cast<u64 *>(p->stacks[1]));
       return 2;
     }
-    k_step<CE, false, true><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, nullptr, nullptr, nullptr, spl);
+    k_step<CE, false, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, nullptr, nullptr, nullptr, spl);
     return 1;
   }
   const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
   if (p->split == 2) {
     u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // collide-stack counters
-    k_step<CE, true, DEV><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+    k_step<CE, true, DEV, EXT><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
                                                           p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, spl);
-    k_collide<CE, DEV><<<cap(G.coll), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], cc, p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
+    k_collide<CE, DEV, EXT><<<cap(G.coll), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], cc, p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
     return 2;
   }
-  k_step<CE, false, DEV><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
+  k_step<CE, false, DEV, EXT><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
                                                          p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, spl);
   return 1;
 }
 
 // the device-driven loop: graph = one WHILE node; body = ONE remap iteration + k_loop_ctl, so the condition (extinct, short
 // enough to drain, error) is tested after every iteration.  Captured once per run on the library's own capture stream.
-template <bool CE>
+template <bool CE, bool EXT>
 static int build_stack_graph(tdr_problem *p, size_t smem) {
   drop_stack_graph(p);
   if (!p->sg_capture) CK(cudaStreamCreateWithFlags(&p->sg_capture, cudaStreamNonBlocking));
@@ -441,10 +441,10 @@ static int build_stack_graph(tdr_problem *p, size_t smem) {
   cudaGraphNode_t node;
   CK(cudaGraphAddNode(&node, p->sg_graph, nullptr, 0, &np));
   cudaGraph_t body = np.conditional.phGraph_out[0];
-  StackGrids G; stack_grids<CE, true>(p, smem, G);
+  StackGrids G; stack_grids<CE, true, EXT>(p, smem, G);
   DevRun none; memset(&none, 0, sizeof none);
   CK(cudaStreamBeginCaptureToGraph(p->sg_capture, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
-  const int per_pass = remap_iteration<CE, true>(p, none, p->sg_capture, smem, G, 0, 1 << 30);
+  const int per_pass = remap_iteration<CE, true, EXT>(p, none, p->sg_capture, smem, G, 0, 1 << 30);
   LoopCtl c; c.ctr = p->ctr; c.R = p->run_dev; c.split = p->split == 1; c.drain_below = (u64)p->drain_below;
   k_loop_ctl<<<1, 32, 0, p->sg_capture>>>(c, h);
   cudaGraph_t captured = nullptr;
@@ -462,7 +462,7 @@ static size_t smem_bytes(const tdr_problem *p) {      // dynamic shared memory =
   return (size_t)p->dp.mg_doubles * sizeof(double) + priv;
 }
 
-template <bool CE>
+template <bool CE, bool EXT>
 static int run_stack(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
   const size_t smem = smem_bytes(p);
@@ -486,8 +486,8 @@ static int run_stack(tdr_problem *p, DevRun R) {
   if ((rc = source(live_stack(0), live_count(0), 0, n0))) return rc;
   u64 n_in = n0;
   StackGrids G;
-  if (dev) { if (!p->sg_exec && (rc = build_stack_graph<CE>(p, smem))) return rc; }
-  else stack_grids<CE, false>(p, smem, G);
+  if (dev) { if (!p->sg_exec && (rc = build_stack_graph<CE, EXT>(p, smem))) return rc; }
+  else stack_grids<CE, false, EXT>(p, smem, G);
   for (;;) {
     R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
     if (dev) {
@@ -503,7 +503,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
       if (cap_blocks < 1) cap_blocks = 1;
       KTimer tb(p, true, 0);                              // one event pair per batch: the launches run back to back
       for (int b = 0; b < batch; b++) {
-        const int nk = remap_iteration<CE, false>(p, R, st, smem, G, it, cap_blocks);
+        const int nk = remap_iteration<CE, false, EXT>(p, R, st, smem, G, it, cap_blocks);
         LAUNCH_CHECK(); p->diag.kernel_launches += nk; p->diag.step_launches += p->time_kernels ? nk : 0;
         it++; p->diag.iterations++;
       }
@@ -527,7 +527,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
       // tail drain: the few particles left are followed to their death in ONE launch (k_drain).  Also under the five-event
       // decomposition: after a whole iteration every survivor waits on the LOOKUP stack, i.e. at the start of a segment.
       const int blocks = (int)((alive + 63) / 64);
-      { KTimer td(p, true); k_drain<CE><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, live_stack(it), live_count(it)); }
+      { KTimer td(p, true); k_drain<CE, EXT><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, live_stack(it), live_count(it)); }
       LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.iterations++;
       CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
       CK(cudaStreamSynchronize(st));
@@ -550,11 +550,11 @@ static int run_stack(tdr_problem *p, DevRun R) {
 }
 
 // ---------------------------------------------------------------------------------- asynchronous scheme, one generation
-template <bool CE, int MODE>
+template <bool CE, int MODE, bool EXT>
 static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int threads) {
-  int grid = grid_for(p, k_async<CE, MODE>, smem, threads);
+  int grid = grid_for(p, k_async<CE, MODE, EXT>, smem, threads);
   KTimer t(p, true);
-  k_async<CE, MODE><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
+  k_async<CE, MODE, EXT><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
                                                         (u32)p->slots_per_warp, p->lockstep, (u32)(p->seg_per_event ? p->seg_per_event : (CE ? 5 : 2)));
   return 0;
 }
@@ -568,7 +568,9 @@ static int run_async(tdr_problem *p, DevRun R) {
   if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
   k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved, p->force_spill ? (1ull << 40) : 0ull);
   LAUNCH_CHECK();
-  if (p->split == 1) launch_async<CE, 1>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2>(p, R, smem, threads); else launch_async<CE, 0>(p, R, smem, threads);
+  const bool ext = p->dp.n_t > 0 || p->dp.implicit;           // the build with the time mesh / weights compiled in (ProbX)
+  if (ext) { if (p->split == 1) launch_async<CE, 1, true>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, true>(p, R, smem, threads); else launch_async<CE, 0, true>(p, R, smem, threads); }
+  else { if (p->split == 1) launch_async<CE, 1, false>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, false>(p, R, smem, threads); else launch_async<CE, 0, false>(p, R, smem, threads); }
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
   u64 *h = p->h_ctr;
   CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
@@ -674,7 +676,11 @@ static int run_generation(tdr_problem *p, DevRun &R) {
   R.sec = p->sec; R.sec_time = p->sec_time; R.sec_w = p->sec_w; R.sec_cap = p->sec_cap; R.sec_limit = 0; R.sec_head0 = 0;
   R.bank = p->bank; R.bank_cap = p->bank_cap;
   R.hist_id = p->hist_id; R.hist_nseg = p->hist_nseg; R.hist_ncoll = p->hist_ncoll;
-  if (p->scheme == 0) { int rc = p->ce ? run_stack<true>(p, R) : run_stack<false>(p, R); return rc ? rc : overflow_check(p); }
+  if (p->scheme == 0) {
+    const bool ext = p->dp.n_t > 0 || p->dp.implicit;
+    int rc = p->ce ? (ext ? run_stack<true, true>(p, R) : run_stack<true, false>(p, R)) : (ext ? run_stack<false, true>(p, R) : run_stack<false, false>(p, R));
+    return rc ? rc : overflow_check(p);
+  }
   { int rc = run_async_any(p, R); return rc ? rc : overflow_check(p); }
 }
 

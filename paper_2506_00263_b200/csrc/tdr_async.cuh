@@ -268,11 +268,13 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R, bool &primary_d
 #ifndef TDR_ASYNC_MINB
 #define TDR_ASYNC_MINB 2
 #endif
-template <bool CE, int MODE>
 #ifndef TDR_ASYNC_MAXT
 #define TDR_ASYNC_MAXT 512
 #endif
-__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P, DevOut O, DevRun R, Soa S, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
+template <bool CE, int MODE, bool EXT>
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut O, DevRun R, Soa S0, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
+  const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
+  const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);

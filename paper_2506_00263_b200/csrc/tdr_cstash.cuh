@@ -124,7 +124,8 @@ __device__ __forceinline__ void cs_push_children_bank(const DevOut &O, const Dev
 }
 
 template <bool CE, int MODE>
-__global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P, DevOut O, DevRun R, PsMem A, int NS, u64 deadline_ns) {
+__global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevOut O, DevRun R, PsMem A, int NS, u64 deadline_ns) {
+  const ProbX<false> &P = static_cast<const ProbX<false> &>(P0);   // the particle stashes run without the time mesh / weights (the host refuses)
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   __shared__ CsCtl ctl;

@@ -35,7 +35,13 @@ struct DevProb {
   const u32 *hash; u32 hash_bmin, hash_n;    // X3: bucket -> first candidate grid index
   double grid_lo, grid_hi;
   u64 n_bins;
+  static constexpr bool EXT = true;            // as a plain DevProb every extension is decided at run time (see ProbX)
 };
+// The time mesh (TD1-TD6) and implicit capture (W1-W4) are extensions most runs do not use; carried as run-time switches they
+// cost the hot kernels registers (time, weight, speed, distance to the time edge).  The hot kernels therefore come in two
+// builds and see the problem and the state through these tag types: with EXT = false the extensions are compiled out (the
+// host launches that build only when n_t == 0 and implicit == 0), with EXT = true they are the run-time switches above.
+template <bool X_> struct ProbX : DevProb { static constexpr bool EXT = X_; };
 // MG row layout: [0] sig_t [1] sig_s_tot [2] sig_c [3] nu*sig_f [4] nu [5..5+G) scatter cdf
 #define MGROW(G) (5 + (G))
 
@@ -50,7 +56,9 @@ struct Soa {                                  // particle state, one array per f
   u32 *seg, *ncoll;
   double *s_sigt, *s_nsf, *s_d, *s_f;        // split-decomposition scratch
   u32 *s_flags, *s_gi;
+  static constexpr bool EXT = true;
 };
+template <bool X_> struct SoaX : Soa { static constexpr bool EXT = X_; };
 
 struct DevRun {
   u64 seed; u32 gen; int kmode, active; double k_prev;
@@ -270,19 +278,19 @@ __device__ __forceinline__ u64 pack_loc1(const Part &p) {
   return (u64)(p.mx & 0xFFFF) | ((u64)(p.my & 0xFFFF) << 16) | ((u64)(p.mz & 0xFFFF) << 32) | ((u64)(p.g & 0xFF) << 48) | ((u64)(p.it & 0xFF) << 56);
 }
 
-template <bool CE>
-__device__ __forceinline__ void load_part(const Soa &s, u32 i, Part &p) {
+template <bool CE, class ST>
+__device__ __forceinline__ void load_part(const ST &s, u32 i, Part &p) {
   p.x = s.x[i]; p.y = s.y[i]; p.z = s.z[i]; p.u = s.u[i]; p.v = s.v[i]; p.w = s.w[i];
-  p.E = CE ? s.E[i] : 0.0; p.t = s.t ? s.t[i] : 0.0; p.wgt = s.wgt ? s.wgt[i] : 1.0;
+  p.E = CE ? s.E[i] : 0.0; p.t = (ST::EXT && s.t) ? s.t[i] : 0.0; p.wgt = (ST::EXT && s.wgt) ? s.wgt[i] : 1.0;
   p.id = s.id[i]; p.seg = s.seg[i]; p.ncoll = s.ncoll[i];
   unpack_loc(p, s.loc0[i], s.loc1[i]);
 }
-template <bool CE>
-__device__ __forceinline__ void store_part(const Soa &s, u32 i, const Part &p) {
+template <bool CE, class ST>
+__device__ __forceinline__ void store_part(const ST &s, u32 i, const Part &p) {
   s.x[i] = p.x; s.y[i] = p.y; s.z[i] = p.z; s.u[i] = p.u; s.v[i] = p.v; s.w[i] = p.w;
   if (CE) s.E[i] = p.E;
-  if (s.t) s.t[i] = p.t;
-  if (s.wgt) s.wgt[i] = p.wgt;
+  if (ST::EXT && s.t) s.t[i] = p.t;
+  if (ST::EXT && s.wgt) s.wgt[i] = p.wgt;
   s.id[i] = p.id; s.seg[i] = p.seg; s.ncoll[i] = p.ncoll;
   s.loc0[i] = pack_loc0(p); s.loc1[i] = pack_loc1(p);
 }

@@ -135,7 +135,8 @@ __device__ __forceinline__ void ev_lookup(const DevProb &P, const double *mg, co
 }
 
 // ---------------------------------------------------------------------------------- T2-T4 MOVE
-__device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Part &p, double St, double &d, u32 &flags) {
+template <class PT>
+__device__ __forceinline__ void ev_move(const PT &P, u64 seed, u32 gen, Part &p, double St, double &d, u32 &flags) {
   p.seg += 1;                                                          // R3
   double dcoll = TDR_INF;
   if (St > 0.0) dcoll = -det_log(draw(seed, p.id, gen, p.seg, PUR_DIST, 0)) / St;
@@ -162,7 +163,7 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   double dmy = (myl == yl && myh == yh) ? dy : plane_dist(myl, myh, p.y, p.v);
   double dmz = (mzl == zl && mzh == zh) ? dz : plane_dist(mzl, mzh, p.z, p.w);
   double vel = 0.0, dtm = TDR_INF;                                    // TD1, TD2: speed, distance to the next time edge
-  if (P.n_t > 0) {
+  if (PT::EXT && P.n_t > 0) {
     vel = P.G > 0 ? P.speed[p.g] : 1.3831592e6 * sqrt(p.E);
     dtm = (P.t_edges[p.it + 1] - p.t) * vel;
   }
@@ -181,14 +182,14 @@ __device__ __forceinline__ void ev_move(const DevProb &P, u64 seed, u32 gen, Par
   if (!(d < TDR_INF)) { flags = F_LOST; d = 0.0; return; }
   if (collide) flags = F_COLLIDE;
   else flags = (dx == d ? F_DX : 0) | (dy == d ? F_DY : 0) | (dz == d ? F_DZ : 0) | (dout == d ? F_DOUT : 0) |
-               (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0) | (dtm == d ? F_TIME : 0);
+               (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0) | ((PT::EXT && dtm == d) ? F_TIME : 0);
   p.x = p.x + d * p.u; p.y = p.y + d * p.v; p.z = p.z + d * p.w;       // G6
-  if (P.n_t > 0) p.t = p.t + d / vel;                                  // TD3
+  if (PT::EXT && P.n_t > 0) p.t = p.t + d / vel;                                  // TD3
 }
 
 // ---------------------------------------------------------------------------------- T5 TALLY (warp-cooperative)
-template <bool CE>
-__device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, const TallyPriv &tp, const DevRun &R, const Part &p, bool valid,
+template <bool CE, class PT>
+__device__ __forceinline__ void ev_tally(const PT &P, const DevOut &o, const TallyPriv &tp, const DevRun &R, const Part &p, bool valid,
                                          double d, double St, double nsf, u32 flags, i64 &accP, i64 &accPc) {
   int e = -1;
   if (valid) {
@@ -204,10 +205,10 @@ __device__ __forceinline__ void ev_tally(const DevProb &P, const DevOut &o, cons
   if (R.kmode && valid) { accP += fixp(d * nsf, P.scale); if (collide && nsf != 0.0) accPc += fixp(nsf / St, P.scale); }
   if (R.active) {
     u64 bin = 0;
-    if (e >= 0) bin = (((((u64)p.it * P.mesh_n[2] + p.mz) * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;     // TD4
+    if (e >= 0) bin = (((((u64)(PT::EXT ? p.it : 0) * P.mesh_n[2] + p.mz) * P.mesh_n[1] + p.my) * P.mesh_n[0]) + p.mx) * P.n_e + e;     // TD4
     // W2: scores carry the weight (identically 1 in analog runs)
-    tally_add(o.flux, tp.flux_lo, tp.flux_hi, tp.n > 0, bin, fixp(P.implicit ? p.wgt * d : d, P.scale), e >= 0);
-    tally_add(o.coll, tp.coll_lo, tp.coll_hi, tp.n > 0, bin, fixp(P.implicit ? p.wgt : 1.0, P.scale), e >= 0 && collide);
+    tally_add(o.flux, tp.flux_lo, tp.flux_hi, tp.n > 0, bin, fixp((PT::EXT && P.implicit) ? p.wgt * d : d, P.scale), e >= 0);
+    tally_add(o.coll, tp.coll_lo, tp.coll_hi, tp.n > 0, bin, fixp((PT::EXT && P.implicit) ? p.wgt : 1.0, P.scale), e >= 0 && collide);
   }
 }
 
@@ -252,8 +253,9 @@ __device__ TDR_COLD void record_deaths_warp(BlockAcc *a, const DevRun &R, bool v
 // "handles weights and weight windows for the particle's next loop iteration": weight roulette below w_roulette.  It runs
 // at the tail of the COLLIDE and SURFACE events (the two that end a segment) under every decomposition; analog runs
 // (weights identically 1) skip it on a uniform branch.
-__device__ __forceinline__ bool ev_closeout(const DevProb &P, const DevRun &R, BlockAcc *acc, Part &p) {
-  if (!P.implicit || !(p.wgt < P.w_roulette)) return true;
+template <class PT>
+__device__ __forceinline__ bool ev_closeout(const PT &P, const DevRun &R, BlockAcc *acc, Part &p) {
+  if (!PT::EXT || !P.implicit || !(p.wgt < P.w_roulette)) return true;
   if (draw(R.seed, p.id, R.gen, p.seg, PUR_CLOSEOUT, 0) * P.w_survive < p.wgt) { p.wgt = P.w_survive; return true; }
   record_death(acc, R, p, TDR_T_NROULETTE);
   return false;
@@ -261,8 +263,8 @@ __device__ __forceinline__ bool ev_closeout(const DevProb &P, const DevRun &R, B
 
 // ---------------------------------------------------------------------------------- T6 COLLIDE
 // returns true if the particle survives; n_children / child_src set on fission
-template <bool CE>
-__device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
+template <bool CE, class PT>
+__device__ __forceinline__ bool ev_collide(const PT &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
                                            double St, int gi, double f, int &n_children, int &child_src) {
   const u64 seed = R.seed; const u32 gen = R.gen;
   n_children = 0; child_src = 0;
@@ -273,7 +275,7 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
     const double *row = mg + (mat * P.G + p.g) * MGROW(P.G);
     double r = draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * St;
     if (r < row[1]) kind = 0; else if (r < row[1] + row[2]) kind = 1; else kind = 2;
-    if (P.implicit) {                                                  // W3: capture by weight, then scatter or fission
+    if (PT::EXT && P.implicit) {                                       // W3: capture by weight, then scatter or fission
       const double snc = St - row[2];
       if (snc > 0.0) { p.wgt = p.wgt * (snc / St); kind = (draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * snc < row[1]) ? 0 : 2; }
       else kind = 1;
@@ -299,7 +301,7 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
     }
     double r2 = blk_odd(sb) * st;
     if (r2 < ss) kind = 0; else if (r2 < ss + sc) kind = 1; else kind = 2;
-    if (P.implicit) {                                                  // W3
+    if (PT::EXT && P.implicit) {                                       // W3
       const double snc = st - sc;
       if (snc > 0.0) { p.wgt = p.wgt * (snc / st); kind = (blk_odd(sb) * snc < ss) ? 0 : 2; }
       else kind = 1;
@@ -318,7 +320,8 @@ __device__ __forceinline__ bool ev_collide(const DevProb &P, const double *mg, c
 }
 
 // ---------------------------------------------------------------------------------- T7 SURFACE (G7)
-__device__ __forceinline__ bool ev_surface(const DevProb &P, const DevRun &R, BlockAcc *acc, Part &p, u32 flags) {
+template <class PT>
+__device__ __forceinline__ bool ev_surface(const PT &P, const DevRun &R, BlockAcc *acc, Part &p, u32 flags) {
   bool alive = true;
   const double u0 = p.u, v0 = p.v, w0 = p.w;
   int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
@@ -360,7 +363,7 @@ __device__ __forceinline__ bool ev_surface(const DevProb &P, const DevRun &R, Bl
     if (a == 0) { p.x = plane; p.mx = idx; } else if (a == 1) { p.y = plane; p.my = idx; } else { p.z = plane; p.mz = idx; }
   }
   if (!alive) record_death(acc, R, p, TDR_T_NLEAK);
-  if (flags & F_TIME) {                                                // TD3: a time edge; the last one is the census
+  if (PT::EXT && (flags & F_TIME)) {                                   // TD3: a time edge; the last one is the census
     p.t = P.t_edges[p.it + 1]; p.it += 1;
     if (p.it == P.n_t && alive) { alive = false; record_death(acc, R, p, TDR_T_NCENSUS); }
   }

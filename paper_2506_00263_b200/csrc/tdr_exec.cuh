@@ -16,8 +16,8 @@ __device__ __forceinline__ void load_loc_energy(const Soa &S, u32 i, Part &p) {
 
 // returns the next event of this lane's particle (NEXT_DEAD if it died or the lane is idle)
 // IO (EV_STEP only): bit 0 = load the particle from the SoA state first, bit 1 = store a survivor back
-template <bool CE, int EV, bool HYBRID = false, int IO = 3>
-__device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, const DevOut &O, const TallyPriv &tp, const DevRun &R, const Soa &S,
+template <bool CE, int EV, bool HYBRID = false, int IO = 3, class PT, class ST>
+__device__ __forceinline__ int exec_event(const PT &P, const double *mg, const DevOut &O, const TallyPriv &tp, const DevRun &R, const ST &S,
                                           BlockAcc *acc, u32 slot, bool valid, Part &p, int &nch, int &csrc,
                                           i64 &accP, i64 &accPc, int first_ev) {
   nch = 0; csrc = 0;
@@ -34,7 +34,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
       if ((flags & F_LOST) || p.seg >= (1u << 24)) atomicExch(O.err, TDR_ELOST);
       else if (flags & F_COLLIDE) {
         if (HYBRID) {                                     // hybrid scheme: collisions are their own event (uniform warps)
-          S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; S.s_sigt[slot] = St; if (S.t) S.t[slot] = p.t;
+          S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; S.s_sigt[slot] = St; if (ST::EXT && S.t) S.t[slot] = p.t;
           if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
           return EV_COLLIDE;
         }
@@ -61,7 +61,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     double d; u32 flags;
     ev_move(P, R.seed, R.gen, p, S.s_sigt[slot], d, flags);
     if ((flags & F_LOST) || p.seg >= (1u << 24)) { atomicExch(O.err, TDR_ELOST); return NEXT_DEAD; }
-    S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; if (S.t) S.t[slot] = p.t;
+    S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; if (ST::EXT && S.t) S.t[slot] = p.t;
     S.s_d[slot] = d; S.s_flags[slot] = flags;
     return EV_TALLY;
   }
@@ -69,7 +69,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     double d = 0.0, St = 0.0, nsf = 0.0; u32 flags = 0;
     if (valid) {
       load_loc_energy<CE>(S, slot, p);
-      p.wgt = S.wgt ? S.wgt[slot] : 1.0;
+      p.wgt = (ST::EXT && S.wgt) ? S.wgt[slot] : 1.0;
       d = S.s_d[slot]; St = S.s_sigt[slot]; nsf = S.s_nsf[slot]; flags = S.s_flags[slot];
     }
     ev_tally<CE>(P, O, tp, R, p, valid, d, St, nsf, flags, accP, accPc);
@@ -84,7 +84,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     if (alive) {
       S.u[slot] = p.u; S.v[slot] = p.v; S.w[slot] = p.w; S.ncoll[slot] = p.ncoll; S.loc1[slot] = pack_loc1(p);
       if (CE) S.E[slot] = p.E;
-      if (S.wgt) S.wgt[slot] = p.wgt;
+      if (ST::EXT && S.wgt) S.wgt[slot] = p.wgt;
     } else if (R.defer_death) S.ncoll[slot] = p.ncoll;
     return alive ? first_ev : NEXT_DEAD;
   }
@@ -94,7 +94,7 @@ __device__ __forceinline__ int exec_event(const DevProb &P, const double *mg, co
     bool alive = ev_surface(P, R, acc, p, S.s_flags[slot]);
     if (alive) {
       S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.u[slot] = p.u; S.v[slot] = p.v; S.w[slot] = p.w;
-      S.loc0[slot] = pack_loc0(p); S.loc1[slot] = pack_loc1(p); if (S.t) S.t[slot] = p.t; if (S.wgt) S.wgt[slot] = p.wgt;
+      S.loc0[slot] = pack_loc0(p); S.loc1[slot] = pack_loc1(p); if (ST::EXT && S.t) S.t[slot] = p.t; if (ST::EXT && S.wgt) S.wgt[slot] = p.wgt;
     }
     return alive ? first_ev : NEXT_DEAD;
   }

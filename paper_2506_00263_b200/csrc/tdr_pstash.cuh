@@ -195,7 +195,8 @@ __device__ __forceinline__ bool ps_birth_from_links(PsWarp &w, const DevProb &P,
 
 // ---------------------------------------------------------------------------------- the persistent kernel
 template <bool CE, int MODE>
-__global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P, DevOut O, DevRun R, PsMem A, int NS, u64 deadline_ns) {
+__global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P0, DevOut O, DevRun R, PsMem A, int NS, u64 deadline_ns) {
+  const ProbX<false> &P = static_cast<const ProbX<false> &>(P0);   // the particle stashes run without the time mesh / weights (the host refuses)
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);

@@ -8,8 +8,10 @@
 
 struct StackSet { u32 *s[EV_COUNT]; u64 *cnt; };      // cnt[e] = device counter of stack e
 
-template <bool CE, int EV, bool DEV>
-__global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, StackSet K, int zero_ev) {
+template <bool CE, int EV, bool DEV, bool EXT>
+__global__ void __launch_bounds__(256) k_event(DevProb P0, DevOut O, DevRun Rv, const DevRun *Rp, Soa S0, StackSet K, int zero_ev) {
+  const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
+  const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   TDR_BIND_RUN(DEV, Rv, Rp)
@@ -44,9 +46,11 @@ __global__ void __launch_bounds__(256) k_event(DevProb P, DevOut O, DevRun Rv, c
 
 // hybrid scheme, second kernel of a remap iteration: the COLLIDE event on the collide stack; survivors (and lanes
 // reborn by make_work) join the step stack the preceding k_step<CE, true> launch was pushing to.
-template <bool CE, bool DEV>
-__global__ void __launch_bounds__(256) k_collide(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, const u32 *cstack, const u64 *ccount,
+template <bool CE, bool DEV, bool EXT>
+__global__ void __launch_bounds__(256) k_collide(DevProb P0, DevOut O, DevRun Rv, const DevRun *Rp, Soa S0, const u32 *cstack, const u64 *ccount,
                                                  u32 *stack_out, u64 *count_out) {
+  const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
+  const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   if (DEV) {                                       // bases in, this iteration's pointers out (see k_step)
     u64 *ctr = const_cast<u64 *>(ccount);
     const u64 it = ctr[C_PENDING];

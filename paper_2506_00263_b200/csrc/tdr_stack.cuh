@@ -139,10 +139,12 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
 // The host-driven loop passes the pointers of its iteration; the device-driven loop passes the bases (stack_in = stack 0,
 // stack_out = stack 1, count_in = the counter block `ctr`) and every kernel derives its own from the iteration counter that
 // k_loop_ctl keeps in ctr[C_PENDING] — so the WHILE body is ONE iteration and the loop condition is tested after each.
-template <bool CE, bool HYBRID, bool DEV>
-__global__ void __launch_bounds__(256, 2) k_step(DevProb P, DevOut O, DevRun Rv, const DevRun *Rp, Soa S, const u32 *stack_in, const u64 *count_in,
+template <bool CE, bool HYBRID, bool DEV, bool EXT>
+__global__ void __launch_bounds__(256, 2) k_step(DevProb P0, DevOut O, DevRun Rv, const DevRun *Rp, Soa S0, const u32 *stack_in, const u64 *count_in,
                                               u32 *stack_out, u64 *count_out, u64 *count_zero,
                                               u32 *cstack, u64 *ccount, u64 *ccount_zero, u32 seg_per_launch) {
+  const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
+  const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   if (DEV) {
     u64 *ctr = const_cast<u64 *>(count_in);
     const u64 it = ctr[C_PENDING];
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(256, 2) k_step(DevProb P, DevOut O, DevRun Rv,
         else if (flags & F_COLLIDE) {
           if (HYBRID) {
             if (k > 0) store_part<CE>(S, slot, p);       // an earlier crossing of this launch changed direction / indices too
-            else { S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; if (S.t) S.t[slot] = p.t; }
+            else { S.x[slot] = p.x; S.y[slot] = p.y; S.z[slot] = p.z; S.seg[slot] = p.seg; if (EXT && S.t) S.t[slot] = p.t; }
             S.s_sigt[slot] = St;
             if (CE) { S.s_gi[slot] = (u32)gi; S.s_f[slot] = f; }
             to_collide = true; alive = false;
@@ -208,8 +210,10 @@ __global__ void __launch_bounds__(256, 2) k_step(DevProb P, DevOut O, DevRun Rv,
 // follows each remaining particle to its death in registers: one launch instead of ~100.  No make_work (nothing is
 // left to claim), children go to the fission bank as usual; a warp keeps calling the warp-cooperative tally until
 // its last lane is done.
-template <bool CE>
-__global__ void __launch_bounds__(256) k_drain(DevProb P, DevOut O, DevRun R, Soa S, const u32 *stack_in, const u64 *count_in) {
+template <bool CE, bool EXT>
+__global__ void __launch_bounds__(256) k_drain(DevProb P0, DevOut O, DevRun R, Soa S0, const u32 *stack_in, const u64 *count_in) {
+  const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
+  const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
