@@ -315,7 +315,7 @@ static u64 layout(tdr_problem *p, u64 n, char *base, bool assign) {
   u64 hist_cap = 16 * (n < 2000000 ? n : 2000000) + 4096;
   u64 *hid = c.take<u64>(hist_cap); u32 *hs = c.take<u32>(hist_cap), *hc = c.take<u32>(hist_cap);
   AsyncMem am; async_layout(c, W, sec_cap, p->arena_links_opt, am);
-  PsMem pm; pstash_layout(c, W, p->arena_links_opt, pm);
+  PsMem pm; pstash_layout(c, W, p->arena_links_opt, p->dp.n_t > 0, p->dp.implicit != 0, pm);
   if (assign) {
     p->W = W; p->soa = s; memcpy(p->stacks, st, sizeof st); p->ctr = ctr; p->run_dev = run_dev; p->out = o;
     p->bank = bank; p->srcbank = src; p->sec = sec; p->sec_time = sec_time; p->sec_w = sec_w; p->bank_cap = bank_cap; p->src_cap = src_cap; p->sec_cap = sec_cap;
@@ -554,7 +554,7 @@ template <bool CE, int MODE, bool EXT>
 static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int threads) {
   int grid = grid_for(p, k_async<CE, MODE, EXT>, smem, threads);
   KTimer t(p, true);
-  k_async<CE, MODE, EXT><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
+  k_async<CE, MODE, EXT><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->pm, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
                                                         (u32)p->slots_per_warp, p->lockstep, (u32)(p->seg_per_event ? p->seg_per_event : (CE ? 5 : 2)));
   return 0;
 }
@@ -564,8 +564,8 @@ static int run_async(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
   const int threads = p->async_threads;
   const size_t smem = smem_bytes(p) + (threads / 32) * (size_t)STASH_WORDS(p->stash_links) * 4;
-  R.defer_death = 1; R.sec_flag = p->am.sec_flag; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
-  if (!R.kmode) CK(cudaMemsetAsync(p->am.sec_flag, 0, p->sec_cap * 8, st));
+  R.defer_death = 1; R.outstanding = p->ctr + C_PENDING; R.slot_next = p->ctr + C_STACK0; R.starved = p->ctr + C_STARVED; R.W = p->W;
+  if (!R.kmode) { k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull); LAUNCH_CHECK(); }   // the links of secondaries
   k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved, p->force_spill ? (1ull << 40) : 0ull);
   LAUNCH_CHECK();
   const bool ext = p->dp.n_t > 0 || p->dp.implicit;           // the build with the time mesh / weights compiled in (ProbX)

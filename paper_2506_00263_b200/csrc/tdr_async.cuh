@@ -8,25 +8,20 @@
 //  * spill / fetch: global links come from one arena; two sets of AQ queues (empty links,
 //    work links), each queue one 64-bit word (head << 32 | tail).  A warp claims a queue by atomicExch with the
 //    null queue, edits the list privately, and swaps it back; nobody ever waits on an owner.
-//  * make_work: a lane whose particle died claims the next source index (or a pending secondary)
+//  * make_work: a lane whose particle died claims a pending secondary (links of site records,
+//    tdr_links.cuh) or the next source index
 //    and is reborn in the same slot; a warp with no runnable link claims up to 32 fresh slots and fills them.
 //  * load balance / termination: a global count of starved warps makes busy warps spill; a global count of
 //    outstanding particles (source not yet dead + secondaries) tells a starved warp when to exit.  The count is
 //    flushed lazily (when a warp goes idle), so a stale zero can only make an idle warp leave early; a warp that
-//    holds work never leaves, and every warp re-checks the source, the secondary ring and the global queues
+//    holds work never leaves, and every warp re-checks the source, its open link of secondaries and the global queues
 //    before it leaves, so no work is stranded.  No grid-wide synchronisation anywhere.
 #pragma once
-#include "tdr_exec.cuh"
-
-#define AQ 32
-#define NULLQ 0xFFFFFFFFFFFFFFFFull
-#define NOLINK 0xFFFFFFFFu
-#define NOSLOT 0xFFFFFFFFu
-
+#include "tdr_links.cuh"
 
 struct GLink { u32 idx[32]; u32 count, ev, next, pad; };
 enum { AC_GWORK = 0, AC_SPILLS, AC_FETCHES, AC_MAKEWORK, AC_EVENTS, AC_DBG = 8, AC_COUNT = 16 };
-struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *actr; u64 *sec_flag; };
+struct AsyncMem { GLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *actr; };
 
 template <class C>
 static void async_layout(C &c, u64 W, u64 sec_cap, u64 n_links_opt, AsyncMem &am) {
@@ -34,45 +29,6 @@ static void async_layout(C &c, u64 W, u64 sec_cap, u64 n_links_opt, AsyncMem &am
   am.links = c.template take<GLink>(am.n_links);
   am.q_empty = c.template take<u64>(AQ); am.q_work = c.template take<u64>(AQ);
   am.actr = c.template take<u64>(AC_COUNT);
-  am.sec_flag = c.template take<u64>(sec_cap);
-}
-
-__device__ __forceinline__ u64 ld_vol(const u64 *p) { return *(const volatile u64 *)p; }
-__device__ __forceinline__ u64 global_ns() { u64 t; asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t)); return t; }
-
-// ---------------------------------------------------------------------------------- global queues (lane 0 only)
-template <class LinkT>
-__device__ __noinline__ void q_deposit(LinkT *links, u64 *qs, u32 i, u64 mine) {
-  for (;;) {
-    u64 cur = atomicExch(&qs[i], NULLQ);                         // claim whatever is there
-    if (cur != NULLQ) {                                          // merge privately: cur ++ mine
-      *(volatile u32 *)&links[(u32)cur].next = (u32)(mine >> 32);
-      mine = (cur & 0xFFFFFFFF00000000ull) | (mine & 0xFFFFFFFFull);
-    }
-    __threadfence();
-    u64 old = atomicExch(&qs[i], mine);                          // swap it back
-    if (old == NULLQ) return;
-    mine = old; i = (i + 1) % AQ;                                // someone deposited meanwhile: place theirs elsewhere
-  }
-}
-
-// A claimed queue looks like an empty one, so `rounds` full scans are made before the set is taken to be empty.
-template <class LinkT>
-__device__ __noinline__ u32 q_pop(LinkT *links, u64 *qs, u32 start, u32 rounds) {
-  for (u32 a = 0; a < AQ * rounds; a++) {
-    u32 i = (start + a) % AQ;
-    if (ld_vol(&qs[i]) == NULLQ) continue;
-    u64 w = atomicExch(&qs[i], NULLQ);
-    if (w == NULLQ) continue;
-    __threadfence();
-    u32 head = (u32)(w >> 32), tail = (u32)w;
-    if (head != tail) {
-      u32 nxt = *(volatile u32 *)&links[head].next;
-      q_deposit(links, qs, i, ((u64)nxt << 32) | tail);
-    }
-    return head;
-  }
-  return NOLINK;
 }
 
 // builds the empty-link queues (arena link i belongs to queue i % AQ, chained in index order) and resets the
@@ -202,35 +158,19 @@ __device__ __forceinline__ void stash_insert(WarpCtx &w, int e, u32 value, bool 
 }
 
 // ---------------------------------------------------------------------------------- make_work
-// Lanes flagged `want` hold a slot with no particle.  Pending secondaries first (fixed source; a record is
-// claimable once its ready flag carries its own ticket), then the primary source.  Returns true if reborn.
+// Lanes flagged `want` hold a slot with no particle.  Fixed source: secondaries first — the warp's open link of site
+// records, then a full link from the global queues (ps_birth_from_links, tdr_links.cuh: a link is published whole, so
+// nobody waits on a writer) — then the primary source.  Returns true if reborn.
 template <bool CE>
-__device__ __forceinline__ bool make_work_async(const DevProb &P, const double *mg, const DevRun &R, const AsyncMem &A, BlockAcc *acc,
-                                                int *err, Part &p, bool want) {
+__device__ __forceinline__ bool make_work_async(const DevProb &P, const double *mg, const DevRun &R, PsWarp &sw, BlockAcc *acc, Part &p, bool want) {
   const u32 lane = threadIdx.x & 31;
   bool reborn = false;
   u32 m = __ballot_sync(FULL, want);
   if (m == 0) return false;
-  const int leader = __ffs(m) - 1;
   if (!R.kmode) {
-    u64 h = 0; u32 got = 0;
-    if (lane == (u32)leader) {
-      const u32 n = (u32)__popc(m);
-      for (;;) {
-        u64 head = ld_vol(R.sec_head), tail = ld_vol(R.sec_tail);
-        if (head >= tail) break;
-        u64 take = tail - head < n ? tail - head : n;
-        if (atomicCAS(R.sec_head, head, head + take) == head) { h = head; got = (u32)take; break; }
-      }
-    }
-    h = __shfl_sync(FULL, h, leader); got = __shfl_sync(FULL, got, leader);
-    const u32 rank = (u32)__popc(m & lanemask_lt());
-    if (want && rank < got) {
-      const u64 idx = h + rank, k = idx % R.sec_cap;
-      bool ok = true;                                              // its writer is between the ticket and the flag
-      while (ld_vol(&A.sec_flag[k]) != idx + 1) { if (*(volatile int *)err) { ok = false; break; } __nanosleep(20); }
-      if (ok) { __threadfence(); tdr_site s = R.sec[k]; birth_site<CE>(P, mg, R, acc, p, s, R.sec_time ? R.sec_time[k] : 0.0, R.sec_w ? R.sec_w[k] : 1.0); reborn = true; }
-    }
+    u32 hint = 0;
+    if (sw.open_count < (u32)__popc(m)) { if (lane == 0) hint = (u32)ld_vol(&sw.A.ctr[PC_GWORK]); hint = __shfl_sync(FULL, hint, 0); }
+    reborn = ps_birth_from_links<CE>(sw, P, mg, R, acc, p, want, hint);
     m = __ballot_sync(FULL, want && !reborn);
     if (m == 0) return reborn;
   }
@@ -251,12 +191,13 @@ __device__ __forceinline__ bool make_work_async(const DevProb &P, const double *
 
 // warp-uniform; `primary_done` is this warp's sticky note that the primary source is exhausted (the cursor only grows),
 // which in k-mode (no secondaries) makes every later call free of global loads
-__device__ __forceinline__ bool source_has_work(const DevRun &R, bool &primary_done) {
+__device__ __forceinline__ bool source_has_work(const DevRun &R, const PsWarp &sw, bool &primary_done) {
   if (primary_done && R.kmode) return false;
+  if (!R.kmode && sw.open_count > 0) return true;
   int yes = 0;
   if ((threadIdx.x & 31) == 0) {
     if (!primary_done) yes = ld_vol(R.src_next) < R.src_total ? 1 : 2;
-    if (yes != 1 && !R.kmode && ld_vol(R.sec_head) < ld_vol(R.sec_tail)) yes |= 1;
+    if (yes != 1 && !R.kmode && ld_vol(&sw.A.ctr[PC_GWORK]) > 0) yes |= 1;
   }
   yes = __shfl_sync(FULL, yes, 0);
   if (yes & 2) primary_done = true;
@@ -272,7 +213,7 @@ __device__ __forceinline__ bool source_has_work(const DevRun &R, bool &primary_d
 #define TDR_ASYNC_MAXT 512
 #endif
 template <bool CE, int MODE, bool EXT>
-__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut O, DevRun R, Soa S0, AsyncMem A, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
+__global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut O, DevRun R, Soa S0, AsyncMem A, PsMem SA, int L, u64 deadline_ns, u32 fresh_max, int lockstep, u32 seg_per_event) {
   const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
   const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
@@ -286,6 +227,8 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
   w.s.idx = stash_mem; w.s.meta = (int *)(stash_mem + 32 * L); w.s.L = L;
   stash_init(w.s, w.lane);
   const Stash &s = w.s;
+  PsWarp sw;                                  // fixed source: the warp's open link of secondaries (site records)
+  sw.A = SA; sw.err = O.err; sw.lane = w.lane; sw.gw = w.gw; sw.open_id = NOLINK; sw.open_count = 0; sw.n_spill = 0; sw.n_fetch = 0;
   constexpr bool SPLIT = MODE == 1;
   const int first_ev = SPLIT ? EV_LOOKUP : EV_STEP;
   i64 accP = 0, accPc = 0, delta = 0;         // delta: outstanding particles not yet flushed (warp-uniform)
@@ -316,7 +259,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
     else {
       // make_work by a starved warp: only a warp that may still grow its pool of slots, or that holds
       // spare ones, asks; the others are refilled through their SOURCE links
-      if ((fresh < fresh_max || __any_sync(FULL, myfree != NOSLOT)) && source_has_work(R, primary_done)) {
+      if ((fresh < fresh_max || __any_sync(FULL, myfree != NOSLOT)) && source_has_work(R, sw, primary_done)) {
         // starved warp: every lane brings a slot (its own spare one, else a fresh one from the window) and claims work
         u32 need = __ballot_sync(FULL, myfree == NOSLOT);
         if (fresh >= fresh_max) need = 0;                       // this warp's pool of slots is large enough
@@ -328,7 +271,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
           if (b != ~0ull && myfree == NOSLOT) { u64 k = b + __popc(need & lanemask_lt()); if (k < R.W) myfree = (u32)k; }
         }
         Part p;
-        bool born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, myfree != NOSLOT);
+        bool born = make_work_async<CE>(P, mg, R, sw, &acc, p, myfree != NOSLOT);
         u32 slot = myfree;
         if (born) { store_part<CE>(S, slot, p); myfree = NOSLOT; }
         n_makework++;
@@ -342,7 +285,9 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
       for (int k = 0; k < n_ev; k++) { const int pl = s.partial(evs[MODE][k]); const int pc = pl >= 0 ? s.cnt(pl) : 0; if (pc > bc) { l = pl; bc = pc; } }
       if (l < 0) {
         if (fetch_link(w)) continue;
-        // nothing anywhere in reach: publish what this warp knows, then leave or wait (no other warp is waited for)
+        // nothing anywhere in reach: publish what this warp knows, then leave or wait (no other warp is waited for).
+        // Secondaries this warp cannot take itself (it holds no free slot) go to the global queues for the others.
+        if (!R.kmode && sw.open_count > 0) ps_open_deposit(sw);
         if (delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
         u64 out = 0; int er = 0;
         if (w.lane == 0) {
@@ -386,7 +331,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
       if (valid) { id = S.id[slot]; sg = S.seg[slot]; nc = S.ncoll[slot]; }
       record_deaths_warp(&acc, R, valid, id, sg, nc);
       bool born = false;
-      if (source_has_work(R, primary_done)) { born = make_work_async<CE>(P, mg, R, A, &acc, O.err, p, valid); n_makework++; }
+      if (source_has_work(R, sw, primary_done)) { born = make_work_async<CE>(P, mg, R, sw, &acc, p, valid); n_makework++; }
       if (born) store_part<CE>(S, slot, p);
       else if (valid && myfree == NOSLOT) myfree = slot;
       stash_insert(w, first_ev, slot, born);
@@ -406,7 +351,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
         int nc1 = 0, cs1 = 0;
         const int nx = exec_event<CE, EV_STEP, false, 0>(P, mg, O, tp, R, S, &acc, slot, live, p, nc1, cs1, accP, accPc, first_ev);
         const u32 ncw = __reduce_add_sync(FULL, (u32)nc1);
-        if (ncw) { push_children(O, R, &acc, p, nc1, cs1); nc_tot += ncw; }
+        if (ncw) { if (R.kmode) push_children(O, R, &acc, p, nc1, cs1); else ps_push_secondaries(sw, R, &acc, p, nc1, cs1); nc_tot += ncw; }
         if (live && nx == NEXT_DEAD) live = false;
         const u32 lm = __ballot_sync(FULL, live);
         if (lm == 0) break;
@@ -422,7 +367,14 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
       delta += (R.kmode ? 0 : (i64)nc_tot) - (i64)__popc(dm);
       if (dm) stash_insert(w, EV_SOURCE, slot, died);
       stash_insert(w, EV_STEP, slot, live);
-      if ((++n_iter & 63u) == 0 && delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+      if ((++n_iter & 63u) == 0) {
+        if (delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+        if (!R.kmode && sw.open_count > 0) {     // load balance: somebody is starved and this warp sits on secondaries
+          u64 st = 0;
+          if (w.lane == 0) st = ld_vol(R.starved);
+          if (__shfl_sync(FULL, st, 0) > 0) ps_open_deposit(sw);
+        }
+      }
       if (!lockstep && s.nfull() >= 2) {          // no lockstep (tail, or switched off): hand a full link to a starved warp
         u64 st = 0;
         if (w.lane == 0) st = ld_vol(R.starved);
@@ -445,7 +397,7 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
     const u32 dm = __ballot_sync(FULL, died);
     if (dm) {                                                   // only STEP / COLLIDE / SURFACE (or a lost particle) get here
       const u32 nc = __reduce_add_sync(FULL, (u32)nch);
-      if (nc) push_children(O, R, &acc, p, nch, csrc);
+      if (nc) { if (R.kmode) push_children(O, R, &acc, p, nch, csrc); else ps_push_secondaries(sw, R, &acc, p, nch, csrc); }
       delta += (R.kmode ? 0 : (i64)nc) - (i64)__popc(dm);     // k-mode children belong to the next generation
       stash_insert(w, EV_SOURCE, slot, died);                   // the slot waits for the SOURCE event
     }
@@ -456,7 +408,14 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
       else if (e == EV_TALLY) { stash_insert(w, EV_COLLIDE, slot, next == EV_COLLIDE); stash_insert(w, EV_SURFACE, slot, next == EV_SURFACE); }
       else stash_insert(w, EV_LOOKUP, slot, next == EV_LOOKUP);
     }
-    if ((++n_iter & 63u) == 0 && delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+    if ((++n_iter & 63u) == 0) {
+      if (delta != 0) { if (w.lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
+      if (!R.kmode && sw.open_count > 0) {
+        u64 st = 0;
+        if (w.lane == 0) st = ld_vol(R.starved);
+        if (__shfl_sync(FULL, st, 0) > 0) ps_open_deposit(sw);
+      }
+    }
     // load balance: a warp is starved and this one holds more than one runnable link -> hand one over
     if (s.nfull() >= 2) {
       u64 st = 0;
@@ -465,7 +424,11 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
       if (st > 0) spill_link(w, s.full(0), 0);
     }
   }
-  if (w.lane == 0) { atomicAdd(&A.actr[AC_EVENTS], (u64)n_events); atomicAdd(&A.actr[AC_MAKEWORK], (u64)n_makework); }
+  if (w.lane == 0) {
+    atomicAdd(&A.actr[AC_EVENTS], (u64)n_events); atomicAdd(&A.actr[AC_MAKEWORK], (u64)n_makework);
+    if (sw.n_spill) atomicAdd(&A.actr[AC_SPILLS], (u64)sw.n_spill);
+    if (sw.n_fetch) atomicAdd(&A.actr[AC_FETCHES], (u64)sw.n_fetch);
+  }
   __syncthreads();
   acc_flush(&acc, O, accP, accPc);
   priv_flush(tp, O);

@@ -20,32 +20,6 @@
 #pragma once
 #include "tdr_async.cuh"
 
-struct SLink { tdr_site s[32]; u32 count, next, pad0, pad1; };      // a global work link of fission-site records
-enum { PC_GWORK = 0, PC_SPILLS, PC_FETCHES, PC_EV_MOVE, PC_EV_COLLIDE, PC_EV_BIRTH, PC_LN_MOVE, PC_LN_COLLIDE, PC_LN_BIRTH,
-       PC_DBG = 10, PC_COUNT = 16 };
-struct PsMem { SLink *links; u64 n_links; u64 *q_empty, *q_work; u64 *ctr; };
-
-template <class C>
-static void pstash_layout(C &c, u64 W, u64 n_links_opt, PsMem &pm) {
-  pm.n_links = n_links_opt ? n_links_opt : W / 32 + 8192;
-  pm.links = c.template take<SLink>(pm.n_links);
-  pm.q_empty = c.template take<u64>(AQ); pm.q_work = c.template take<u64>(AQ);
-  pm.ctr = c.template take<u64>(PC_COUNT);
-}
-
-__global__ void k_ps_init(PsMem A, u64 *outstanding, u64 n_source, u64 *starved, u64 starved0) {
-  const u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x, nt = (u64)gridDim.x * blockDim.x;
-  for (u64 i = t; i < A.n_links; i += nt) A.links[i].next = (i + AQ < A.n_links) ? (u32)(i + AQ) : NOLINK;
-  if (t < AQ) {
-    const u64 q = t;
-    u64 last = A.n_links > q ? q + ((A.n_links - 1 - q) / AQ) * AQ : 0;
-    A.q_empty[q] = A.n_links > q ? ((q << 32) | last) : NULLQ;
-    A.q_work[q] = NULLQ;
-  }
-  if (t < PC_COUNT) A.ctr[t] = 0;
-  if (t == 0) { *outstanding = n_source; *starved = starved0; }
-}
-
 // ---------------------------------------------------------------------------------- the per-warp pool
 #define PS_RING 128                       // ring capacity (slot numbers are bytes); NS <= PS_RING
 enum { PF_X = 0, PF_Y, PF_Z, PF_U, PF_V, PF_W, PF_ID, PF_L0, PF_L1, PF_E, PF_ST, PF_F };
@@ -88,103 +62,6 @@ struct PsRing {                           // warp-uniform head / count in regist
     return s;
   }
 };
-
-__device__ __forceinline__ tdr_site load_site_cg(const tdr_site *p) {       // written by another SM: bypass L1
-  const ulonglong2 *q = (const ulonglong2 *)p;
-  union { tdr_site s; ulonglong2 v[3]; } r;
-  r.v[0] = __ldcg(q); r.v[1] = __ldcg(q + 1); r.v[2] = __ldcg(q + 2);
-  return r.s;
-}
-
-struct PsWarp {                           // warp-uniform runtime state
-  PsMem A; int *err; u32 lane, gw;
-  u32 open_id, open_count;                // the global link this warp is filling with secondaries (private until deposited)
-  u32 n_spill, n_fetch;
-};
-
-__device__ __forceinline__ bool ps_open_acquire(PsWarp &w) {
-  u32 g = NOLINK;
-  if (w.lane == 0) g = q_pop(w.A.links, w.A.q_empty, w.gw, 256);
-  g = __shfl_sync(FULL, g, 0);
-  if (g == NOLINK) { if (w.lane == 0) atomicExch(w.err, TDR_ECAPACITY); return false; }
-  w.open_id = g; w.open_count = 0;
-  return true;
-}
-
-// publish the open link whole: it enters a work queue only when every record in it is written
-__device__ __forceinline__ void ps_open_deposit(PsWarp &w) {
-  if (w.open_id == NOLINK || w.open_count == 0) return;
-  __syncwarp();
-  if (w.lane == 0) {
-    w.A.links[w.open_id].count = w.open_count; w.A.links[w.open_id].next = NOLINK;
-    __threadfence();
-    q_deposit(w.A.links, w.A.q_work, w.gw % AQ, ((u64)w.open_id << 32) | w.open_id);
-    atomicAdd(&w.A.ctr[PC_GWORK], 1ull);
-  }
-  __syncwarp();
-  w.n_spill++; w.open_id = NOLINK; w.open_count = 0;
-}
-
-// fixed source: n fission secondaries per lane (T6) -> site records in the warp's open link; full links are deposited
-__device__ TDR_COLD void ps_push_secondaries(PsWarp &w, const DevRun &R, BlockAcc *acc, const Part &p, int n, int src) {
-  const u32 total = __reduce_add_sync(FULL, (u32)n);
-  if (total == 0) return;
-  u32 incl = (u32)n;
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) { const u32 t = __shfl_up_sync(FULL, incl, o); if (w.lane >= (u32)o) incl += t; }
-  const u32 excl = incl - (u32)n;
-  if (w.lane == 0) acc_add(acc, TDR_T_NSITES, (u64)total);
-  u32 done = 0;
-  while (done < total) {
-    if (w.open_id == NOLINK && !ps_open_acquire(w)) return;
-    const u32 take = min(32u - w.open_count, total - done);
-    for (int c = 0; c < n; c++) {
-      const u32 o = excl + (u32)c;
-      if (o >= done && o < done + take) w.A.links[w.open_id].s[w.open_count + (o - done)] = make_site(R, p, src, (u32)c);
-    }
-    w.open_count += take; done += take;
-    if (w.open_count == 32) ps_open_deposit(w);
-  }
-  __syncwarp();
-}
-
-// SOURCE event of a fixed-source run: secondaries BEFORE new source particles (depth first), so the links in flight stay
-// bounded by what the resident particles produce however long the source is.  Lanes [0, n) of the warp hold a free slot.
-// (1) the warp's open link, newest record first; (2) when it runs dry and full links wait in the global queues, one of
-// them becomes the open link (the fetch of PAPER.md:87, 95: claimed whole, so nobody waits on a writer) and serves the
-// rest.  Returns true for a lane that was born from a site; gwork_hint is cleared when the queues in reach were empty.
-template <bool CE>
-__device__ __forceinline__ bool ps_birth_from_links(PsWarp &w, const DevProb &P, const double *mg, const DevRun &R, BlockAcc *acc, Part &p,
-                                                    u32 n, u32 &gwork_hint) {
-  bool born = false; u32 served = 0;
-  for (int round = 0; round < 2; round++) {
-    const u32 t = min(n - served, w.open_count);
-    if (t) {
-      if (w.lane >= served && w.lane < served + t) {
-        const tdr_site s = load_site_cg(&w.A.links[w.open_id].s[w.open_count - t + (w.lane - served)]);
-        birth_site<CE>(P, mg, R, acc, p, s); born = true;
-      }
-      w.open_count -= t; served += t;
-    }
-    if (served == n || round == 1 || gwork_hint == 0) break;
-    u32 g = NOLINK;                                  // the open link is empty here
-    if (w.lane == 0) g = q_pop(w.A.links, w.A.q_work, w.gw, 4);
-    g = __shfl_sync(FULL, g, 0);
-    if (g == NOLINK) { gwork_hint = 0; break; }
-    const u32 c = __ldcg(&w.A.links[g].count);
-    if (w.lane == 0) {
-      atomicAdd(&w.A.ctr[PC_GWORK], ~0ull);
-      if (w.open_id != NOLINK) {                     // hand the old (empty) open link back
-        *(volatile u32 *)&w.A.links[w.open_id].next = NOLINK;
-        __threadfence();
-        q_deposit(w.A.links, w.A.q_empty, w.gw % AQ, ((u64)w.open_id << 32) | w.open_id);
-      }
-    }
-    __syncwarp();
-    w.open_id = g; w.open_count = c; w.n_fetch++;
-  }
-  return born;
-}
 
 #ifndef PS_THREADS
 #define PS_THREADS 256
@@ -271,7 +148,7 @@ __global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P0, DevO
       Part p; bool born = false;
       if (!R.kmode) {                                             // (1), (2): secondaries first
         if (w.open_count < n) { u32 g = 0; if (lane == 0) g = (u32)ld_vol(&A.ctr[PC_GWORK]); gwork_hint = __shfl_sync(FULL, g, 0); }
-        born = ps_birth_from_links<CE>(w, P, mg, R, &acc, p, n, gwork_hint);
+        born = ps_birth_from_links<CE>(w, P, mg, R, &acc, p, want, gwork_hint);
       }
       const u32 m = __ballot_sync(FULL, want && !born);           // (3) the primary source: one atomic per warp
       if (m && !primary_done) {

@@ -12,10 +12,6 @@ enum { C_SRC_NEXT = 0, C_SEC_TAIL, C_SEC_HEAD, C_BANK, C_HIST, C_NEXT_BANK, C_PE
 // event ids (split decomposition; async scheme)
 enum { EV_LOOKUP = 0, EV_MOVE, EV_TALLY, EV_COLLIDE, EV_SURFACE, EV_STEP, EV_SOURCE, EV_COUNT };
 
-// asynchronous scheme: a claimed secondary may still be read this many records behind the tail, so the ring keeps
-// this much headroom (>= the number of resident threads, 148 x 2048)
-#define SEC_MARGIN (1ull << 19)
-
 __device__ __forceinline__ u32 lanemask_lt() { u32 m; asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m)); return m; }
 
 // warp-collective push of one index per flagged lane
@@ -29,7 +25,8 @@ __device__ __forceinline__ void stack_push(u32 *stack, u64 *count, u32 value, bo
   if (pred) stack[base + __popc(m & lanemask_lt())] = value;
 }
 
-// warp-collective push of n sites per lane into the fission bank (k-mode) or the secondary ring (fixed source)
+// warp-collective push of n sites per lane into the fission bank (k-mode) or the stack scheme's secondary ring (fixed source;
+// the asynchronous scheme sends its secondaries through links of site records instead: tdr_links.cuh)
 __device__ TDR_COLD void push_children(const DevOut &O, const DevRun &R, BlockAcc *acc, const Part &p, int n, int src) {
   u32 lane = threadIdx.x & 31;
   u32 total = __reduce_add_sync(FULL, (u32)n);
@@ -45,13 +42,9 @@ __device__ TDR_COLD void push_children(const DevOut &O, const DevRun &R, BlockAc
     u64 t = base + excl + c;
     tdr_site s = make_site(R, p, src, (u32)c);
     if (R.kmode) { if (t < R.bank_cap) R.bank[t] = s; else atomicExch(O.err, TDR_ECAPACITY); }
-    else if (!R.sec_flag) { if (t - R.sec_head0 < R.sec_cap) { R.sec[t % R.sec_cap] = s; if (R.sec_time) R.sec_time[t % R.sec_cap] = p.t; if (R.sec_w) R.sec_w[t % R.sec_cap] = p.wgt; } else atomicExch(O.err, TDR_ECAPACITY); }
-    else {                                                       // asynchronous scheme: publish with a ready flag
-      const u64 k = t % R.sec_cap;
-      if ((i64)(t - *(const volatile u64 *)R.sec_head) < (i64)(R.sec_cap - SEC_MARGIN)) {     // the head may already be past t
-        R.sec[k] = s; if (R.sec_time) R.sec_time[k] = p.t; if (R.sec_w) R.sec_w[k] = p.wgt; __threadfence(); *(volatile u64 *)&R.sec_flag[k] = t + 1;
-      } else atomicExch(O.err, TDR_ECAPACITY);
-    }
+    else if (t - R.sec_head0 < R.sec_cap) {                      // stack scheme: the ring; claimable once the loop control has seen the tail
+      R.sec[t % R.sec_cap] = s; if (R.sec_time) R.sec_time[t % R.sec_cap] = p.t; if (R.sec_w) R.sec_w[t % R.sec_cap] = p.wgt;
+    } else atomicExch(O.err, TDR_ECAPACITY);
   }
 }
 
