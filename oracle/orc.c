@@ -159,6 +159,43 @@ double orc_dist_cyl(double X, double Y, double u, double v, double R, int inside
   return d;
 }
 
+/* C2: the surface function; a point with f < 0 is on the negative side (inside a sphere or cylinder) */
+double orc_surf_eval(int kind, const double *co, double X, double Y, double Z) {
+  if (kind == 0) return ((co[0] * X + co[1] * Y) + co[2] * Z) - co[3];
+  const double ox = X - co[0], oy = Y - co[1];
+  if (kind == 1) { const double oz = Z - co[2]; return ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3]; }
+  return (ox * ox + oy * oy) - co[3] * co[3];
+}
+
+/* C3: distance along (u,v,w) to the surface for a particle KNOWN to be on the given side (the side comes from the cell's
+ * definition, not from the sign of f: a particle that has just crossed sits on the surface up to rounding).  Plane: reachable
+ * only when moving towards it.  Sphere / cylinder: G4's two roots with the full quadratic. */
+double orc_surf_dist(int kind, const double *co, double X, double Y, double Z, double u, double v, double w, int negative_side) {
+  double d;
+  if (kind == 0) {
+    const double den = (co[0] * u + co[1] * v) + co[2] * w;
+    if (negative_side ? !(den > 0.0) : !(den < 0.0)) return INFINITY;
+    d = (co[3] - ((co[0] * X + co[1] * Y) + co[2] * Z)) / den;
+  } else {
+    const double ox = X - co[0], oy = Y - co[1], oz = kind == 1 ? Z - co[2] : 0.0, wz = kind == 1 ? w : 0.0;
+    const double a = (u * u + v * v) + wz * wz;
+    if (a == 0.0) return INFINITY;
+    const double b = (ox * u + oy * v) + oz * wz;
+    const double c = ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3];
+    double disc = b * b - a * c;
+    if (negative_side) {
+      if (disc < 0.0) disc = 0.0;
+      d = (-b + sqrt(disc)) / a;
+    } else {
+      if (b >= 0.0) return INFINITY;
+      if (disc <= 0.0) return INFINITY;
+      d = (-b - sqrt(disc)) / a;
+    }
+  }
+  if (d < 0.0) d = 0.0;
+  return d;
+}
+
 /* X2: largest i with grid[i] <= E (E clamped to the grid), capped at n-2 */
 int32_t orc_grid_index(const double *grid, int32_t n, double E) {
   if (E < grid[0]) E = grid[0];
@@ -180,6 +217,7 @@ struct orc_problem {
   int implicit; double w_roulette, w_survive;                                /* W: implicit capture + roulette */
   double *xp, *yp, *zp, *cx, *cy, *univ_rad, *mesh[3], *e_edges, *t_edges, *speed;
   int32_t *cell_univ, *univ_nr, *univ_mat;
+  int n_surf, n_cell; int32_t *surf_kind, *univ_cell0, *univ_ncell, *cell_nsurf, *cell_surf, *cell_mat; double *surf_coef;   /* C: general cells */
   int src_kind, src_dir_kind, src_energy_kind, src_index;
   double src_lo[3], src_hi[3], src_dir[3], src_energy, scale;
   int n_mat, G;
@@ -221,6 +259,7 @@ void orc_free_problem(orc_problem *p) {
   free(p->xp); free(p->yp); free(p->zp); free(p->cx); free(p->cy); free(p->univ_rad);
   for (int a = 0; a < 3; a++) free(p->mesh[a]);
   free(p->e_edges); free(p->t_edges); free(p->speed); free(p->cell_univ); free(p->univ_nr); free(p->univ_mat);
+  free(p->surf_kind); free(p->univ_cell0); free(p->univ_ncell); free(p->cell_nsurf); free(p->cell_surf); free(p->cell_mat); free(p->surf_coef);
   free(p->sig_t); free(p->sig_f); free(p->nu); free(p->sst); free(p->sig_c); free(p->scdf);
   free(p->chicdf); free(p->nusigf); free(p->mat_nnuc); free(p->mat_nuc); free(p->mat_dens);
   free(p->grid); free(p->A); free(p->xs_s); free(p->xs_c); free(p->xs_f); free(p->nuc_nu);
@@ -252,8 +291,23 @@ int orc_init_problem(const orc_geometry *g, const orc_materials *m, const orc_xs
     p->mesh_n[a] = g->mesh_n[a]; p->mesh[a] = DUPD(mp[a], g->mesh_n[a] + 1);
     if (!(p->mesh[a][0] <= lp[a][0]) || !(p->mesh[a][g->mesh_n[a]] >= lp[a][ln[a]])) { orc_free_problem(p); return ORC_EINVAL; }
   }
-  for (int u = 0; u < g->n_univ; u++)
-    if (p->univ_nr[u] < 0 || p->univ_nr[u] > ORC_MAX_RINGS) { orc_free_problem(p); return ORC_EINVAL; }
+  p->n_surf = g->n_surf; p->n_cell = g->n_cell;
+  if (p->n_surf > 0) {
+    if (!g->surf_kind || !g->surf_coef || !g->univ_cell0 || !g->univ_ncell || !g->cell_nsurf || !g->cell_surf || !g->cell_mat || g->n_cell < 1) { orc_free_problem(p); return ORC_EINVAL; }
+    p->surf_kind = DUPI(g->surf_kind, g->n_surf); p->surf_coef = DUPD(g->surf_coef, 4 * g->n_surf);
+    p->univ_cell0 = DUPI(g->univ_cell0, g->n_univ); p->univ_ncell = DUPI(g->univ_ncell, g->n_univ);
+    p->cell_nsurf = DUPI(g->cell_nsurf, g->n_cell); p->cell_surf = DUPI(g->cell_surf, g->n_cell * ORC_MAX_CSURF); p->cell_mat = DUPI(g->cell_mat, g->n_cell);
+    for (int k = 0; k < g->n_surf; k++) if (p->surf_kind[k] < 0 || p->surf_kind[k] > 2 || (p->surf_kind[k] > 0 && !(p->surf_coef[4 * k + 3] > 0.0))) { orc_free_problem(p); return ORC_EINVAL; }
+    for (int k = 0; k < g->n_cell; k++) {
+      if (p->cell_nsurf[k] < 1 || p->cell_nsurf[k] > ORC_MAX_CSURF || p->cell_mat[k] < 0 || p->cell_mat[k] >= m->n_mat) { orc_free_problem(p); return ORC_EINVAL; }
+      for (int j = 0; j < p->cell_nsurf[k]; j++) { int r = p->cell_surf[k * ORC_MAX_CSURF + j]; if (r == 0 || abs(r) > g->n_surf) { orc_free_problem(p); return ORC_EINVAL; } }
+    }
+  }
+  for (int u = 0; u < g->n_univ; u++) {
+    if (p->univ_nr[u] == -1 && p->n_surf > 0) {
+      if (p->univ_cell0[u] < 0 || p->univ_ncell[u] < 1 || p->univ_ncell[u] > 255 || p->univ_cell0[u] + p->univ_ncell[u] > p->n_cell) { orc_free_problem(p); return ORC_EINVAL; }
+    } else if (p->univ_nr[u] < 0 || p->univ_nr[u] > ORC_MAX_RINGS) { orc_free_problem(p); return ORC_EINVAL; }
+  }
   p->G = m->G; p->n_mat = m->n_mat; p->by_group = g->by_group;
   if (p->G > 0) p->n_e = g->by_group ? p->G : 1;
   else { if (g->n_ebins < 1) { orc_free_problem(p); return ORC_EINVAL; } p->n_e = g->n_ebins; p->e_edges = DUPD(g->e_edges, g->n_ebins + 1); }
@@ -347,6 +401,40 @@ static int locate_ring(const orc_problem *p, int univ, double X, double Y) {
   return nr;
 }
 
+/* C4: the cell of a general universe that holds the point: the first cell all of whose half-spaces hold.  A surface in
+ * `crossed` (bit j = surface slot j of cell `from`) is not evaluated: the particle has just gone through it, so it is on
+ * the side opposite to the one cell `from` names.  -1: no cell (undefined geometry). */
+static int locate_cell(const orc_problem *p, int univ, double X, double Y, double Z, int from, unsigned crossed) {
+  const int c0 = p->univ_cell0[univ], nc = p->univ_ncell[univ];
+  for (int k = 0; k < nc; k++) {
+    const int cell = c0 + k; int ok = 1;
+    for (int j = 0; j < p->cell_nsurf[cell] && ok; j++) {
+      const int r = p->cell_surf[cell * ORC_MAX_CSURF + j], sf = abs(r) - 1, want_neg = r < 0;
+      int neg = -1;
+      if (from >= 0)
+        for (int i = 0; i < p->cell_nsurf[from]; i++) {
+          const int rf = p->cell_surf[from * ORC_MAX_CSURF + i];
+          if ((crossed >> i & 1u) && abs(rf) - 1 == sf) neg = !(rf < 0);
+        }
+      if (neg < 0) neg = orc_surf_eval(p->surf_kind[sf], p->surf_coef + 4 * sf, X, Y, Z) < 0.0;
+      ok = neg == want_neg;
+    }
+    if (ok) return k;
+  }
+  return -1;
+}
+
+/* ring (or cell) of a point in a universe, by coordinates (G2, C4) */
+static int locate_in_universe(const orc_problem *p, int univ, double X, double Y, double Z) {
+  if (p->univ_nr[univ] < 0) return locate_cell(p, univ, X, Y, Z, -1, 0u);
+  return locate_ring(p, univ, X, Y);
+}
+
+static int material_of(const orc_problem *p, int univ, int ring) {
+  if (p->univ_nr[univ] < 0) return p->cell_mat[p->univ_cell0[univ] + ring];
+  return p->univ_mat[univ * (ORC_MAX_RINGS + 1) + ring];
+}
+
 static int sample_cdf(const double *cdf, int n, double xi) {   /* X1 */
   double t = xi * cdf[n - 1];
   for (int k = 0; k < n; k++) if (t < cdf[k]) return k;
@@ -391,7 +479,8 @@ static void birth_primary(ctx *c, part *q, uint64_t i) {                /* i = s
   q->mx = find_bin(p->mesh[0], p->mesh_n[0], q->x); q->my = find_bin(p->mesh[1], p->mesh_n[1], q->y);
   q->mz = find_bin(p->mesh[2], p->mesh_n[2], q->z);
   int univ = p->cell_univ[((size_t)q->iz * p->ny + q->iy) * p->nx + q->ix];
-  q->ring = locate_ring(p, univ, q->x - p->cx[q->ix], q->y - p->cy[q->iy]);
+  q->ring = locate_in_universe(p, univ, q->x - p->cx[q->ix], q->y - p->cy[q->iy], q->z);
+  if (q->ring < 0) { c->err = ORC_ELOST; q->ring = 0; }
   birth_common(c, q, 0, 0);
 }
 
@@ -429,7 +518,7 @@ static void transport(ctx *c, part *q) {
     q->seg += 1;                                                        /* R3 */
     const uint32_t seg = q->seg;
     int univ = p->cell_univ[((size_t)q->iz * p->ny + q->iy) * p->nx + q->ix];
-    int mat = p->univ_mat[univ * (ORC_MAX_RINGS + 1) + q->ring];
+    int mat = material_of(p, univ, q->ring);
     /* T1 */
     double St = 0.0, nsf = 0.0;
     double ss[ORC_MAX_NUC], sc[ORC_MAX_NUC], sf[ORC_MAX_NUC], st[ORC_MAX_NUC];
@@ -466,6 +555,15 @@ static void transport(ctx *c, part *q) {
       if (q->ring < nr) dout = orc_dist_cyl(X, Y, u0, v0, p->univ_rad[univ * ORC_MAX_RINGS + q->ring], 1);
       if (q->ring > 0) din = orc_dist_cyl(X, Y, u0, v0, p->univ_rad[univ * ORC_MAX_RINGS + q->ring - 1], 0);
     }
+    double dcs[ORC_MAX_CSURF]; int ncs = 0, gcell = -1;                 /* C5: the surfaces of the current general cell */
+    if (nr < 0) {
+      gcell = p->univ_cell0[univ] + q->ring; ncs = p->cell_nsurf[gcell];
+      const double X = q->x - p->cx[q->ix], Y = q->y - p->cy[q->iy];
+      for (int j = 0; j < ncs; j++) {
+        const int r = p->cell_surf[gcell * ORC_MAX_CSURF + j], sf = abs(r) - 1;
+        dcs[j] = orc_surf_dist(p->surf_kind[sf], p->surf_coef + 4 * sf, X, Y, q->z, u0, v0, w0, r < 0);
+      }
+    }
     double dmx = plane_dist(p->mesh[0][q->mx], p->mesh[0][q->mx + 1], q->x, u0);
     double dmy = plane_dist(p->mesh[1][q->my], p->mesh[1][q->my + 1], q->y, v0);
     double dmz = plane_dist(p->mesh[2][q->mz], p->mesh[2][q->mz + 1], q->z, w0);
@@ -479,6 +577,7 @@ static void transport(ctx *c, part *q) {
     if (dz < ds) ds = dz;
     if (dout < ds) ds = dout;
     if (din < ds) ds = din;
+    for (int j = 0; j < ncs; j++) if (dcs[j] < ds) ds = dcs[j];
     if (dmx < ds) ds = dmx;
     if (dmy < ds) ds = dmy;
     if (dmz < ds) ds = dmz;
@@ -595,8 +694,17 @@ static void transport(ctx *c, part *q) {
       if (din == d) q->ring -= 1;
       if (moved_xy || moved_z) {
         int nu2 = p->cell_univ[((size_t)q->iz * p->ny + q->iy) * p->nx + q->ix];
-        if (moved_xy) q->ring = p->univ_nr[nu2];
+        if (p->univ_nr[nu2] < 0) { if (moved_xy || nu2 != univ) q->ring = locate_in_universe(p, nu2, q->x - p->cx[q->ix], q->y - p->cy[q->iy], q->z); }
+        else if (moved_xy) q->ring = p->univ_nr[nu2];
         else if (nu2 != univ) q->ring = locate_ring(p, nu2, q->x - p->cx[q->ix], q->y - p->cy[q->iy]);
+        if (q->ring < 0) { c->err = ORC_ELOST; return; }
+      } else if (ncs > 0) {                                             /* C6: through one or more surfaces of a general cell */
+        unsigned crossed = 0u;
+        for (int j = 0; j < ncs; j++) if (dcs[j] == d) crossed |= 1u << j;
+        if (crossed) {
+          q->ring = locate_cell(p, univ, q->x - p->cx[q->ix], q->y - p->cy[q->iy], q->z, gcell, crossed);
+          if (q->ring < 0) { c->err = ORC_ELOST; return; }
+        }
       }
       if (dmx == d) { if (u0 > 0.0) { q->x = p->mesh[0][q->mx + 1]; if (q->mx + 1 < p->mesh_n[0]) q->mx += 1; } else { q->x = p->mesh[0][q->mx]; if (q->mx > 0) q->mx -= 1; } }
       if (dmy == d) { if (v0 > 0.0) { q->y = p->mesh[1][q->my + 1]; if (q->my + 1 < p->mesh_n[1]) q->my += 1; } else { q->y = p->mesh[1][q->my]; if (q->my > 0) q->my -= 1; } }

@@ -30,6 +30,7 @@ extern "C" {
 
 #define ORC_MAX_RINGS 4
 #define ORC_MAX_NUC 4
+#define ORC_MAX_CSURF 6
 
 enum { ORC_OK = 0, ORC_EINVAL = -1, ORC_ENOMEM = -2, ORC_ECAPACITY = -4, ORC_ELOST = -5,
        ORC_EOVERFLOW = -6, ORC_ESTATE = -7 };
@@ -61,6 +62,17 @@ typedef struct orc_geometry {
   const double *t_edges;                     /* n_tbins+1 ascending; t_edges[0] = emission time, t_edges[n_tbins] = census */
   int32_t implicit_capture;                  /* fixed source: capture by weight reduction + weight roulette (the closeout event) */
   double w_roulette, w_survive;              /* roulette below w_roulette; survivors get w_survive */
+  /* general cells (readings C1-C6): a universe with univ_nrings[u] == -1 is a list of cells, each the
+   * intersection of up to ORC_MAX_CSURF half-spaces of surfaces given in the frame of the lattice cell
+   * (X = x - cx[ix], Y = y - cy[iy], Z = z); the particle's `ring` then holds its cell within the universe */
+  int32_t n_surf;
+  const int32_t *surf_kind;                  /* n_surf: 0 plane aX + bY + cZ = d; 1 sphere centre (a,b,c) radius d; 2 z-cylinder axis (a,b) radius d */
+  const double *surf_coef;                   /* n_surf*4: a, b, c, d */
+  int32_t n_cell;
+  const int32_t *univ_cell0, *univ_ncell;    /* n_univ: first cell / number of cells (<= 255) of a general universe */
+  const int32_t *cell_nsurf;                 /* n_cell: 1..ORC_MAX_CSURF */
+  const int32_t *cell_surf;                  /* n_cell*ORC_MAX_CSURF: +(s+1) = the side f_s >= 0, -(s+1) = the side f_s < 0 */
+  const int32_t *cell_mat;                   /* n_cell */
 } orc_geometry;
 
 typedef struct orc_materials {
@@ -137,6 +149,9 @@ double orc_watt(uint64_t seed, uint64_t id, uint32_t gen, double a, double b);
 void orc_scatter_ce(uint64_t seed, uint64_t id, uint32_t gen, uint32_t seg, double A, double E,
                     const double dir_in[3], double *E_out, double dir_out[3]);
 double orc_dist_cyl(double X, double Y, double u, double v, double R, int inside);
+/* readings C2, C3: value of the surface function (negative inside) and distance to the surface from the given side */
+double orc_surf_eval(int kind, const double *coef, double X, double Y, double Z);
+double orc_surf_dist(int kind, const double *coef, double X, double Y, double Z, double u, double v, double w, int negative_side);
 int32_t orc_grid_index(const double *grid, int32_t n, double E);
 
 #ifdef __cplusplus

@@ -44,7 +44,9 @@ class Geometry(C.Structure):
                 ("src_dir_kind", C.c_int32), ("src_dir", C.c_double * 3),
                 ("src_energy_kind", C.c_int32), ("src_index", C.c_int32), ("src_energy", C.c_double),
                 ("tally_scale_log2", C.c_int32), ("n_tbins", C.c_int32), ("t_edges", PD),
-                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double)]
+                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double),
+                ("n_surf", C.c_int32), ("surf_kind", PI), ("surf_coef", PD), ("n_cell", C.c_int32), ("univ_cell0", PI), ("univ_ncell", PI),
+                ("cell_nsurf", PI), ("cell_surf", PI), ("cell_mat", PI)]
 
 
 class Materials(C.Structure):
@@ -104,6 +106,10 @@ def lib():
         L.orc_scatter_ce.restype = None
         L.orc_dist_cyl.argtypes = [C.c_double, C.c_double, C.c_double, C.c_double, C.c_double, C.c_int]
         L.orc_dist_cyl.restype = C.c_double
+        L.orc_surf_eval.argtypes = [C.c_int, PD, C.c_double, C.c_double, C.c_double]
+        L.orc_surf_eval.restype = C.c_double
+        L.orc_surf_dist.argtypes = [C.c_int, PD] + [C.c_double] * 6 + [C.c_int]
+        L.orc_surf_dist.restype = C.c_double
         L.orc_grid_index.argtypes = [PD, C.c_int32, C.c_double]
         L.orc_grid_index.restype = C.c_int32
         _lib = L

@@ -31,7 +31,7 @@ enum { CE_MOVE = 0, CE_COLLIDE = 1, CE_BIRTH = 2, CE_IDLE = 3, CE_EXIT = 4 };
 struct CsCtl {                              // CTA-wide scheduler state in shared memory
   u32 tail[3], head[3];                     // monotonically increasing counters; ring index = counter & mask
   u32 ev, base, n;                          // the round descriptor
-  u32 primary_done, open_total, reaping, gwork_hint, starved, backoff, rounds, arrived;
+  u32 primary_done, open_total, reaping, gwork_hint, starved, backoff, rounds;
   unsigned long long t_idle, last_out, t_start;
 };
 
@@ -123,51 +123,6 @@ __device__ __forceinline__ void cs_push_children_bank(const DevOut &O, const Dev
   }
 }
 
-// The scheduler of a CTA's rounds, run by ONE lane (of the warp that finished the previous round last): picks the event type
-// whose ring holds the most work, fixes the range of ring entries the round consumes and publishes both in ctl.
-__device__ __forceinline__ void cs_decide(CsCtl &ctl, const DevRun &R, const PsMem &A, const DevOut &O, u32 cap, u64 deadline_ns) {
-  if (ctl.ev == CE_IDLE) {
-    // the idle round has published every warp's outstanding count: leave if the whole run is done, else wait for links from
-    // busy CTAs (nobody in particular is waited for)
-    const u64 out = ld_vol(R.outstanding); const int er = *(volatile int *)O.err;
-    const u64 now = global_ns();
-    if (out != ctl.last_out) { ctl.last_out = out; ctl.t_idle = now; }
-    else if (now - ctl.t_idle > deadline_ns) atomicExch(O.err, TDR_ELOST);
-    if (out == 0 || er != 0 || now - ctl.t_idle > deadline_ns) ctl.reaping = 1;
-    else {
-      if (!ctl.starved) { ctl.starved = 1; atomicAdd(R.starved, 1ull); }
-      __nanosleep(ctl.backoff); if (ctl.backoff < 4000) ctl.backoff += ctl.backoff;
-    }
-  }
-  const u32 cM = ctl.tail[CE_MOVE] - ctl.head[CE_MOVE], cC = ctl.tail[CE_COLLIDE] - ctl.head[CE_COLLIDE], cB = ctl.tail[CE_BIRTH] - ctl.head[CE_BIRTH];
-  bool can_birth = !ctl.primary_done;
-  if (!R.kmode) {
-    // a look at the global queues (one L2 round trip) before any round that could be a birth round: full links are taken
-    // BEFORE new source particles (depth first), so the links in flight stay bounded by what the resident particles
-    // produce however long the source is; once the source is exhausted, the look decides whether births are possible
-    const bool birth_in_reach = can_birth ? (cB >= cap || (cB > cM && cB > cC)) : (ctl.open_total == 0 && cB >= 32 && cM + cC < cap);
-    if (birth_in_reach) ctl.gwork_hint = (u32)ld_vol(&A.ctr[PC_GWORK]);
-    if (!can_birth) can_birth = ctl.open_total > 0 || (cB >= 32 && ctl.gwork_hint > 0);
-  }
-  // hard watchdog (a scheduler that stopped making progress must end in an error code, not in a hung device)
-  if ((++ctl.rounds & 4095u) == 0 && !ctl.reaping && global_ns() - ctl.t_start > 4 * deadline_ns) { atomicExch(O.err, TDR_ELOST); ctl.reaping = 1; }
-  u32 ev;
-  if (ctl.reaping) ev = cB > 0 ? CE_BIRTH : CE_EXIT;
-  else if (cC >= cap) ev = CE_COLLIDE;
-  else if (cM >= cap) ev = CE_MOVE;
-  else if (cB >= cap && can_birth) ev = CE_BIRTH;
-  else if (cM + cC > 0) ev = (can_birth && cB > cM && cB > cC) ? CE_BIRTH : (cC > cM ? CE_COLLIDE : CE_MOVE);
-  else if (cB > 0 && can_birth) ev = CE_BIRTH;
-  else if (R.kmode) { ctl.reaping = 1; ev = CE_BIRTH; }       // nothing left: book the remaining deaths, then leave
-  else ev = CE_IDLE;
-  if (ev <= CE_BIRTH) {
-    const u32 c = ev == CE_MOVE ? cM : ev == CE_COLLIDE ? cC : cB;
-    ctl.base = ctl.head[ev]; ctl.n = c < cap ? c : cap; ctl.head[ev] += ctl.n;
-    if (ctl.starved) { ctl.starved = 0; ctl.backoff = 250; atomicAdd(R.starved, ~0ull); }
-  }
-  ctl.ev = ev;
-}
-
 template <bool CE, int MODE>
 __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevOut O, DevRun R, PsMem A, int NS, u64 deadline_ns) {
   const ProbX<false> &P = static_cast<const ProbX<false> &>(P0);   // the particle stashes run without the time mesh / weights (the host refuses)
@@ -184,7 +139,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
     for (int r = 0; r < 3; r++) { ctl.tail[r] = 0; ctl.head[r] = 0; }
     ctl.tail[CE_BIRTH] = (u32)NS;
     ctl.primary_done = 0; ctl.open_total = 0; ctl.reaping = 0; ctl.gwork_hint = 0; ctl.starved = 0; ctl.backoff = 250;
-    ctl.t_idle = 0; ctl.last_out = ~0ull; ctl.rounds = 0; ctl.t_start = global_ns(); ctl.arrived = 0; ctl.ev = CE_MOVE;
+    ctl.t_idle = 0; ctl.last_out = ~0ull; ctl.rounds = 0; ctl.t_start = global_ns();
   }
   acc_init(&acc);                             // (ends with a barrier)
   PsWarp w;
@@ -192,19 +147,57 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
   w.open_id = NOLINK; w.open_count = 0; w.n_spill = 0; w.n_fetch = 0;
   i64 accP = 0, accPc = 0, delta = 0;
   u32 ev_cnt[3] = { 0, 0, 0 }, ln_cnt[3] = { 0, 0, 0 }, open_pub = 0;
-  if (threadIdx.x == 0) cs_decide(ctl, R, A, O, cap, deadline_ns);       // the first round
-  __syncthreads();
   for (;;) {
-    // the round descriptor was written before the barrier the warps just left; nobody writes it again before they have all
-    // arrived at the end of this round
+    __syncthreads();                          // A: every push of the last round is in the rings
+    if (threadIdx.x == 0) {
+      const u32 cM = ctl.tail[CE_MOVE] - ctl.head[CE_MOVE], cC = ctl.tail[CE_COLLIDE] - ctl.head[CE_COLLIDE], cB = ctl.tail[CE_BIRTH] - ctl.head[CE_BIRTH];
+      bool can_birth = !ctl.primary_done;
+      if (!R.kmode) {
+        // a look at the global queues (one L2 round trip) before any round that could be a birth round: full links are taken
+        // BEFORE new source particles (depth first), so the links in flight stay bounded by what the resident particles
+        // produce however long the source is; once the source is exhausted, the look decides whether births are possible
+        const bool birth_in_reach = can_birth ? (cB >= cap || (cB > cM && cB > cC)) : (ctl.open_total == 0 && cB >= 32 && cM + cC < cap);
+        if (birth_in_reach) ctl.gwork_hint = (u32)ld_vol(&A.ctr[PC_GWORK]);
+        if (!can_birth) can_birth = ctl.open_total > 0 || (cB >= 32 && ctl.gwork_hint > 0);
+      }
+      // hard watchdog (a scheduler that stopped making progress must end in an error code, not in a hung device)
+      if ((++ctl.rounds & 4095u) == 0 && !ctl.reaping && global_ns() - ctl.t_start > 4 * deadline_ns) { atomicExch(O.err, TDR_ELOST); ctl.reaping = 1; }
+      u32 ev;
+      if (ctl.reaping) ev = cB > 0 ? CE_BIRTH : CE_EXIT;
+      else if (cC >= cap) ev = CE_COLLIDE;
+      else if (cM >= cap) ev = CE_MOVE;
+      else if (cB >= cap && can_birth) ev = CE_BIRTH;
+      else if (cM + cC > 0) ev = (can_birth && cB > cM && cB > cC) ? CE_BIRTH : (cC > cM ? CE_COLLIDE : CE_MOVE);
+      else if (cB > 0 && can_birth) ev = CE_BIRTH;
+      else if (R.kmode) { ctl.reaping = 1; ev = CE_BIRTH; }       // nothing left: book the remaining deaths, then leave
+      else ev = CE_IDLE;
+      if (ev <= CE_BIRTH) {
+        const u32 c = ev == CE_MOVE ? cM : ev == CE_COLLIDE ? cC : cB;
+        ctl.base = ctl.head[ev]; ctl.n = c < cap ? c : cap; ctl.head[ev] += ctl.n;
+        if (ctl.starved) { ctl.starved = 0; ctl.backoff = 250; atomicAdd(R.starved, ~0ull); }
+      }
+      ctl.ev = ev;
+    }
+    __syncthreads();                          // B: the round descriptor is published
     const u32 ev = ctl.ev;
     if (ev == CE_EXIT) break;
-    do {
     if (ev == CE_IDLE) {
-      // fixed source, nothing in the stash and nothing to claim: every warp publishes its count of outstanding particles; the
-      // warp that decides the next round then looks at the global count (cs_decide)
+      // fixed source, nothing in the stash and nothing to claim: publish this CTA's count of outstanding particles, then
+      // leave if the whole run is done, else wait for links from busy CTAs (nobody in particular is waited for)
       if (delta != 0) { if (lane == 0) atomicAdd(R.outstanding, (u64)delta); delta = 0; }
-      break;
+      __syncthreads();
+      if (threadIdx.x == 0) {
+        const u64 out = ld_vol(R.outstanding); const int er = *(volatile int *)O.err;
+        const u64 now = global_ns();
+        if (out != ctl.last_out) { ctl.last_out = out; ctl.t_idle = now; }
+        else if (now - ctl.t_idle > deadline_ns) atomicExch(O.err, TDR_ELOST);
+        if (out == 0 || er != 0 || now - ctl.t_idle > deadline_ns) ctl.reaping = 1;
+        else {
+          if (!ctl.starved) { ctl.starved = 1; atomicAdd(R.starved, 1ull); }
+          __nanosleep(ctl.backoff); if (ctl.backoff < 4000) ctl.backoff += ctl.backoff;
+        }
+      }
+      continue;
     }
     const u32 my = wid * 32;
     const u32 n = ctl.n > my ? min(32u, ctl.n - my) : 0u;
@@ -216,7 +209,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
         if (lane == 0) atomicAdd(&ctl.open_total, 0u - open_pub);
         open_pub = 0;
       }
-      break;
+      continue;
     }
     const bool valid = lane < n;
     const u32 slot = valid ? (u32)pl.ring[ev][(ctl.base + my + lane) & pl.mask] : 0u;
@@ -230,7 +223,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
         if (dead) { id = pl.q[PF_ID * NS + slot]; sg = pl.w[slot]; nc = pl.w[NS + slot]; pl.w[slot] = CS_FRESH; }
         record_deaths_warp(&acc, R, dead, id, sg, nc);
       }
-      if (ctl.reaping) break;
+      if (ctl.reaping) continue;
       Part p; bool born = false;
       if (!R.kmode) {                                             // (1), (2): secondaries first (the warp's open link, then the global queues)
         u32 hint = ctl.gwork_hint;
@@ -256,7 +249,7 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
       pl.push3(&ctl, slot, born, false, valid && !born);
       if (!R.kmode && w.open_count != open_pub) { if (lane == 0) atomicAdd(&ctl.open_total, w.open_count - open_pub); open_pub = w.open_count; }
       ev_cnt[CE_BIRTH]++; ln_cnt[CE_BIRTH] += __popc(__ballot_sync(FULL, born));
-      break;
+      continue;
     }
 
     if (ev == CE_MOVE) {
@@ -320,14 +313,6 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
         }
       }
     }
-    } while (0);
-    // one barrier per round: the warp that arrives LAST decides the next round (all pushes of this round are behind their
-    // warps' arrivals), while the others already wait at the barrier
-    __syncwarp();
-    int last = 0;
-    if (lane == 0) { __threadfence_block(); last = atomicAdd(&ctl.arrived, 1u) == nw - 1; }
-    if (__shfl_sync(FULL, last, 0) && lane == 0) { ctl.arrived = 0; cs_decide(ctl, R, A, O, cap, deadline_ns); }
-    __syncthreads();
   }
   if (delta != 0 && lane == 0) atomicAdd(R.outstanding, (u64)delta);
   if (lane == 0) {

@@ -149,13 +149,10 @@ __device__ __forceinline__ double det_log(double x) {
 __device__ __forceinline__ i64 fixp(double v, double scale) { return __double2ll_rn(v * scale); }   // N5
 
 // ---------------------------------------------------------------------------------- B2 / B3 / T6 samplers
-// b0 = the block of attempt 0, computed by the caller next to its other blocks: independent Philox chains issued together
-// overlap their fixed latencies (the path is bound by dependent-issue stalls, profiles/ncu_r02.md)
-__device__ __forceinline__ int iso_dir(const Blk &b0, u64 seed, u64 id, u32 gen, u32 seg, double &u, double &v, double &w) {
-  Blk b = b0;
+__device__ __forceinline__ int iso_dir(u64 seed, u64 id, u32 gen, u32 seg, double &u, double &v, double &w) {
 #pragma unroll 1
   for (u32 a = 0; a < MAX_ATTEMPT; a++) {
-    if (a) b = rng_block(seed, id, gen, seg, PUR_DIR, a);
+    Blk b = rng_block(seed, id, gen, seg, PUR_DIR, a);
     double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;
     double s = v1 * v1 + v2 * v2;
     if (s < 1.0) {
@@ -184,17 +181,16 @@ __device__ __forceinline__ double watt(u64 seed, u64 id, u32 gen, double a, doub
   return (W + aab / 4.0) + (2.0 * x2 - 1.0) * sqrt(aab * W);
 }
 
-__device__ __forceinline__ void scatter_ce(const Blk &ben, const Blk &bdir0, u64 seed, u32 gen, Part &p, double A) {
+__device__ __forceinline__ void scatter_ce(u64 seed, u32 gen, Part &p, double A) {
   double u = p.u, v = p.v, w = p.w;
-  double mu = 2.0 * blk_even(ben) - 1.0;
+  double mu = 2.0 * draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0) - 1.0;
   double q = (A * A + (2.0 * A) * mu) + 1.0;
   p.E = p.E * (q / ((A + 1.0) * (A + 1.0)));
   double mul = (1.0 + A * mu) / sqrt(q);
   double cphi = 1.0, sphi = 0.0;
-  Blk b = bdir0;
 #pragma unroll 1
   for (u32 t = 0; t < MAX_ATTEMPT; t++) {
-    if (t) b = rng_block(seed, p.id, gen, p.seg, PUR_DIR, t);
+    Blk b = rng_block(seed, p.id, gen, p.seg, PUR_DIR, t);
     double v1 = 2.0 * blk_even(b) - 1.0, v2 = 2.0 * blk_odd(b) - 1.0;
     double s = v1 * v1 + v2 * v2;
     if (s < 1.0 && s > 0.0) { cphi = (v1 * v1 - v2 * v2) / s; sphi = (2.0 * v1 * v2) / s; break; }

@@ -143,9 +143,7 @@ __device__ __forceinline__ void ev_move(const PT &P, u64 seed, u32 gen, Part &p,
   const double xl = P.xp[p.ix], xh = P.xp[p.ix + 1], yl = P.yp[p.iy], yh = P.yp[p.iy + 1], zl = P.zp[p.iz], zh = P.zp[p.iz + 1];
   double dx = plane_dist(xl, xh, p.x, p.u);
   double dy = plane_dist(yl, yh, p.y, p.v);
-  // an axis along which no lane of the warp can reach a plane (a lattice infinite in z: cfg1, cfg3, cfg4) skips its division
-  double dz = TDR_INF;
-  if (p.w != 0.0 && fabs((p.w > 0.0 ? zh : zl) - p.z) < TDR_INF) dz = plane_dist(zl, zh, p.z, p.w);
+  double dz = plane_dist(zl, zh, p.z, p.w);
   double dout = TDR_INF, din = TDR_INF;
   int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
   int nr = P.univ_nr[univ];
@@ -273,27 +271,23 @@ __device__ __forceinline__ bool ev_collide(const PT &P, const double *mg, const 
   p.ncoll += 1;
   int univ; int mat = cell_material(P, p, univ);
   int kind; double nu;
-  // the three blocks every scattering collision needs, issued together (a capture or a fission wastes two of them, at no
-  // cost in issue slots as long as one lane of the warp scatters)
-  const Blk bsel = rng_block(seed, p.id, gen, p.seg, PUR_SELECT, 0), ben = rng_block(seed, p.id, gen, p.seg, PUR_ENERGY, 0),
-            bdir0 = rng_block(seed, p.id, gen, p.seg, PUR_DIR, 0);
   if (!CE) {
     const double *row = mg + (mat * P.G + p.g) * MGROW(P.G);
-    double r = blk_odd(bsel) * St;
+    double r = draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * St;
     if (r < row[1]) kind = 0; else if (r < row[1] + row[2]) kind = 1; else kind = 2;
     if (PT::EXT && P.implicit) {                                       // W3: capture by weight, then scatter or fission
       const double snc = St - row[2];
-      if (snc > 0.0) { p.wgt = p.wgt * (snc / St); kind = (blk_odd(bsel) * snc < row[1]) ? 0 : 2; }
+      if (snc > 0.0) { p.wgt = p.wgt * (snc / St); kind = (draw(seed, p.id, gen, p.seg, PUR_SELECT, 1) * snc < row[1]) ? 0 : 2; }
       else kind = 1;
     }
     nu = row[4]; child_src = mat;
     if (kind == 0) {
-      p.g = sample_cdf(row + 5, P.G, blk_even(ben));
-      if (iso_dir(bdir0, seed, p.id, gen, p.seg, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
+      p.g = sample_cdf(row + 5, P.G, draw(seed, p.id, gen, p.seg, PUR_ENERGY, 0));
+      if (iso_dir(seed, p.id, gen, p.seg, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
       return ev_closeout(P, R, acc, p);
     }
   } else {
-    const Blk &sb = bsel;
+    Blk sb = rng_block(seed, p.id, gen, p.seg, PUR_SELECT, 0);
     double r = blk_even(sb) * St;
     int nn = P.mat_nnuc[mat];
     double acc_s = 0.0, ss = 0.0, sc = 0.0, st = 0.0; int nuc = 0;
@@ -313,7 +307,7 @@ __device__ __forceinline__ bool ev_collide(const PT &P, const double *mg, const 
       else kind = 1;
     }
     nu = P.nuc_nu[nuc]; child_src = nuc;
-    if (kind == 0) { scatter_ce(ben, bdir0, seed, gen, p, P.A[nuc]); return ev_closeout(P, R, acc, p); }
+    if (kind == 0) { scatter_ce(seed, gen, p, P.A[nuc]); return ev_closeout(P, R, acc, p); }
   }
   if (kind == 1) { record_death(acc, R, p, TDR_T_NABS); return false; }
   double nu_eff = R.kmode ? nu / R.k_prev : nu;
@@ -382,7 +376,7 @@ __device__ __forceinline__ void birth_common(const DevProb &P, const double *mg,
                                              int src, bool from_site) {
   p.seg = 0; p.ncoll = 0; p.E = 0.0; p.g = 0;
   if (!from_site && P.src_dir_kind == 1) { p.u = P.src_dir[0]; p.v = P.src_dir[1]; p.w = P.src_dir[2]; }
-  else if (iso_dir(rng_block(R.seed, p.id, R.gen, 0, PUR_DIR, 0), R.seed, p.id, R.gen, 0, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
+  else if (iso_dir(R.seed, p.id, R.gen, 0, p.u, p.v, p.w)) acc_add(acc, TDR_T_NDIRFAIL, 1ull);
   if (from_site) {
     if (!CE) p.g = sample_cdf(mg + P.n_mat * P.G * MGROW(P.G) + src * P.G, P.G, draw(R.seed, p.id, R.gen, 0, PUR_ENERGY, 0));
     else p.E = watt(R.seed, p.id, R.gen, P.wa[src], P.wb[src]);

@@ -16,6 +16,7 @@ import numpy as np
 
 MAX_RINGS = 4
 MAX_NUC = 4
+MAX_CSURF = 6
 PROBLEM_SEED = 0x25060263
 INF = float("inf")
 
@@ -44,18 +45,27 @@ def _i32(a):
 
 def geometry(xplanes, yplanes, zplanes, cell_univ, universes, bc, mesh=None, by_group=0,
              e_edges=None, src_kind=0, src_lo=(0, 0, 0), src_hi=(0, 0, 0), src_dir=None,
-             src_energy=("group", 0), scale_log2=24, cx=None, cy=None, t_edges=None, implicit=None):
-    """universes: list of (radii ascending, materials innermost..background)."""
+             src_energy=("group", 0), scale_log2=24, cx=None, cy=None, t_edges=None, implicit=None, surfaces=None):
+    """universes: list of (radii ascending, materials innermost..background), or ("cells", [(signed surfaces, material), ...]) for a
+    universe of general cells (readings C1-C6): each cell is the intersection of half-spaces of `surfaces`
+    = [(kind, a, b, c, d)], kind "plane" | "sphere" | "zcyl", named +(s+1) for the side f >= 0 and -(s+1) for f < 0."""
     xp, yp, zp = _f64(xplanes), _f64(yplanes), _f64(zplanes)
     nx, ny, nz = len(xp) - 1, len(yp) - 1, len(zp) - 1
     if cx is None:
         cx = [0.5 * (xp[i] + xp[i + 1]) if np.isfinite(xp[i]) and np.isfinite(xp[i + 1]) else 0.0 for i in range(nx)]
     if cy is None:
         cy = [0.5 * (yp[i] + yp[i + 1]) if np.isfinite(yp[i]) and np.isfinite(yp[i + 1]) else 0.0 for i in range(ny)]
-    nr = _i32([len(u[0]) for u in universes])
+    nr = _i32([-1 if u[0] == "cells" else len(u[0]) for u in universes])
     rad = np.zeros((len(universes), MAX_RINGS))
     mat = np.zeros((len(universes), MAX_RINGS + 1), dtype=np.int32)
+    cell0, ncell, cell_ns, cell_sf, cell_mat = np.zeros(len(universes), np.int32), np.zeros(len(universes), np.int32), [], [], []
     for k, (radii, mats) in enumerate(universes):
+        if radii == "cells":
+            cell0[k], ncell[k] = len(cell_ns), len(mats)
+            for sf, m in mats:
+                assert 1 <= len(sf) <= MAX_CSURF and all(r != 0 and abs(r) <= len(surfaces) for r in sf)
+                cell_ns.append(len(sf)); cell_sf.append(list(sf) + [0] * (MAX_CSURF - len(sf))); cell_mat.append(m)
+            continue
         assert len(mats) == len(radii) + 1 and len(radii) <= MAX_RINGS
         rad[k, :len(radii)] = radii
         mat[k, :len(mats)] = mats
@@ -78,6 +88,11 @@ def geometry(xplanes, yplanes, zplanes, cell_univ, universes, bc, mesh=None, by_
              n_tbins=(len(t_edges) - 1 if t_edges is not None else 0), t_edges=_f64(t_edges if t_edges is not None else [0.0]),
              implicit_capture=0 if implicit is None else 1, w_roulette=0.0 if implicit is None else float(implicit[0]),
              w_survive=0.0 if implicit is None else float(implicit[1]))
+    if surfaces:
+        kinds = {"plane": 0, "sphere": 1, "zcyl": 2}
+        g.update(n_surf=len(surfaces), surf_kind=_i32([kinds[t[0]] for t in surfaces]), surf_coef=_f64([list(t[1:5]) for t in surfaces]),
+                 n_cell=len(cell_ns), univ_cell0=_i32(cell0), univ_ncell=_i32(ncell), cell_nsurf=_i32(cell_ns), cell_surf=_i32(cell_sf),
+                 cell_mat=_i32(cell_mat))
     return g
 
 
@@ -180,6 +195,39 @@ def two_region(kind="pin", n=200000, seed=1):
         geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((R1, R), (1, 0, 1))], [1, 1, 1, 1, 0, 0],
                        src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0))
         frac = pi * (R * R - R1 * R1) / (4 * h * h)
+    elif kind in ("sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells"):
+        # general cells (readings C1-C6): "fuel" (material 0) is a cell, or several, of a universe of general cells
+        c = 1.0                                                # half width of the cube; z is finite here (spheres)
+        box = dict(bc=[1] * 6, src_kind=1, src_lo=(-c, -c, -c), src_hi=(c, c, c))
+        if kind == "sphere":                                   # a sphere off the cell centre
+            surf = [("sphere", 0.1, -0.2, 0.15, 0.7)]
+            cells = [((-1,), 0), ((+1,), 1)]
+            frac = 4.0 / 3.0 * pi * 0.7 ** 3 / 8.0
+        elif kind == "halfspace":                              # an oblique plane X + 2Y + 2Z = 0.9 (unit normal times 3)
+            surf = [("plane", 1.0, 2.0, 2.0, 0.9)]
+            cells = [((-1,), 0), ((+1,), 1)]
+            frac = None                                        # by quadrature in the test
+        elif kind == "offcyl":                                 # a z-cylinder whose axis is not the cell's
+            surf = [("zcyl", 0.25, -0.3, 0.0, 0.6)]
+            cells = [((+1,), 1), ((-1,), 0)]                   # (cell order must not matter)
+            frac = pi * 0.36 * 2.0 / 8.0
+        elif kind == "shell":                                  # fuel = the shell between two concentric spheres, cut by a plane
+            surf = [("sphere", 0.0, 0.0, 0.0, 0.4), ("sphere", 0.0, 0.0, 0.0, 0.9), ("plane", 0.0, 0.0, 1.0, 0.0)]
+            cells = [((-1,), 1), ((+1, -2, +3), 0), ((+1, -2, -3), 1), ((+2,), 1)]
+            frac = 0.5 * 4.0 / 3.0 * pi * (0.9 ** 3 - 0.4 ** 3) / 8.0
+        elif kind == "lens":                                   # fuel = the intersection of two spheres (two surfaces met at once on its rim)
+            surf = [("sphere", -0.3, 0.0, 0.0, 0.7), ("sphere", 0.3, 0.0, 0.0, 0.7)]
+            cells = [((-1, -2), 0), ((-1, +2), 1), ((+1, -2), 1), ((+1, +2), 1)]
+            hcap = 0.7 - 0.3
+            frac = 2.0 * (pi * hcap * hcap * (3 * 0.7 - hcap) / 3.0) / 8.0
+        else:                                                  # 2 x 2 lattice: general cells next to a ring universe
+            surf = [("sphere", 0.0, 0.0, 0.0, 0.45)]
+            cells = [((-1,), 0), ((+1,), 1)]
+            geo = geometry([-1.0, 0.0, 1.0], [-1.0, 0.0, 1.0], [-0.5, 0.5], [0, 1, 1, 0], [("cells", cells), ((0.3,), (0, 1))], [1] * 6,
+                           src_kind=1, src_lo=(-1.0, -1.0, -0.5), src_hi=(1.0, 1.0, 0.5), surfaces=surf)
+            frac = (2 * 4.0 / 3.0 * pi * 0.45 ** 3 + 2 * pi * 0.09 * 1.0) / 4.0
+        if kind != "lattice_cells":
+            geo = geometry([-c, c], [-c, c], [-c, c], [0], [("cells", cells)], surfaces=surf, **box)
     else:
         raise ValueError(kind)
     p = Problem("two_region_" + kind, geo, mats, None, "fixed", n, seed=seed)

@@ -498,3 +498,65 @@ def test_implicit_capture_with_fission_chains(ce):
     assert abs(r["flux"].sum() / S24 / n - ref) < 0.03 * ref and abs(a["flux"].sum() / S24 / n - ref) < 0.03 * ref
     T = r["totals"]
     assert T["n_abs"] == 0 and T["n_born"] == n + T["n_sites"] == T["n_fis"] + T["n_roulette"]
+
+
+# ------------------------------------------------------------------ C: general cells (readings C1-C6)
+def _halfspace_fraction():
+    """Volume fraction of the cube [-1, 1]^3 with X + 2 Y + 2 Z < 0.9, by quadrature (independent of the oracle)."""
+    g = np.linspace(-1, 1, 2001); g = 0.5 * (g[1:] + g[:-1])
+    Y, Z = np.meshgrid(g, g, indexing="ij")
+    xmax = np.clip(0.9 - 2 * Y - 2 * Z, -1, 1)                 # X runs from -1 to xmax
+    return float(np.mean(xmax + 1) / 2)
+
+
+@pytest.mark.parametrize("kind", ["sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells"])
+def test_general_cells_split_a_flat_flux_by_volume(kind):
+    """The flat-flux volume pin on universes of general cells: a wrong root or side in the distance to a sphere, plane or
+    cylinder, a cell search that ignores the crossed surface, a missed tie on the rim of the lens or a missed re-location at a
+    lattice plane moves the share of absorptions in the fuel cells by many sigma (or loses particles)."""
+    n = 200000
+    p = W.two_region(kind, n=n)
+    r = orc.run(p)
+    T = r["totals"]
+    assert T["n_born"] == n and T["n_leak"] == 0 and T["n_fis"] + T["n_abs"] == n
+    f = p.notes["fuel_volume_fraction"] if kind != "halfspace" else _halfspace_fraction()
+    assert abs(T["n_fis"] / n - f) < 4 * math.sqrt(f * (1 - f) / n), (kind, T["n_fis"] / n, f)
+    assert abs(r["flux"][0] / S24 / n - 1 / 0.3) < 4 * (1 / 0.3) / math.sqrt(n)
+    assert T["n_cross"] > n / 2
+
+
+def test_surface_distance_lands_on_the_surface_and_is_the_first_hit():
+    """orc_surf_dist against a brute-force march of the surface function (sign changes of orc_surf_eval along the ray), for
+    all three kinds from both sides."""
+    rng = np.random.default_rng(11)
+    PDc = C.POINTER(C.c_double)
+    for kind, co in ((0, [0.3, -0.5, 0.8, 0.2]), (1, [0.1, -0.2, 0.3, 0.9]), (2, [-0.2, 0.1, 0.0, 0.7])):
+        ca = (C.c_double * 4)(*co)
+        hits = 0
+        for _ in range(300):
+            r0 = rng.uniform(-1.5, 1.5, 3); d = rng.normal(size=3); d /= np.linalg.norm(d)
+            f0 = L.orc_surf_eval(kind, ca, *r0)
+            neg = f0 < 0
+            dist = L.orc_surf_dist(kind, ca, *r0, *d, int(neg))
+            ts = np.linspace(0, 6, 6001)[1:]
+            fs = np.array([L.orc_surf_eval(kind, ca, *(r0 + t * d)) for t in ts])
+            change = np.nonzero((fs < 0) != neg)[0]
+            if len(change) == 0:
+                assert dist == math.inf or dist > 6 - 2e-3, (kind, r0, d, dist)
+                continue
+            hits += 1
+            assert abs(dist - ts[change[0]]) < 2e-3, (kind, r0, d, dist, ts[change[0]])
+            assert abs(L.orc_surf_eval(kind, ca, *(r0 + dist * d))) < 1e-9
+        assert hits > 50
+
+
+def test_sphere_of_absorber_in_a_void_transmits_exp_minus_sigma_r():
+    """A point source at the centre of a purely absorbing sphere (S = 1.3, R = 0.8) inside a void with vacuum faces: the
+    share that leaks is exp(-S R) whatever the direction (pins the outward root and the cell change sphere -> void)."""
+    n, S, R = 100000, 1.3, 0.8
+    geo = W.geometry([-2, 2], [-2, 2], [-2, 2], [0], [("cells", [((-1,), 0), ((+1,), 1)])], [0] * 6, surfaces=[("sphere", 0.0, 0.0, 0.0, R)])
+    mats = W.mg_materials([[S], [0.0]], [[[0.0]], [[0.0]]], [[0.0], [0.0]], [[0.0], [0.0]], [[1.0], [1.0]])
+    r = orc.run(W.Problem("sphere_void", geo, mats, None, "fixed", n))
+    t = math.exp(-S * R)
+    assert abs(r["totals"]["n_leak"] / n - t) < 4 * math.sqrt(t * (1 - t) / n)
+    assert r["totals"]["n_cross"] >= r["totals"]["n_leak"] * 2                # sphere surface, then the box face
