@@ -27,6 +27,7 @@ extern "C" {
 
 #define TDR_MAX_RINGS 4
 #define TDR_MAX_NUC 4
+#define TDR_MAX_CSURF 6
 
 enum { TDR_OK = 0, TDR_EINVAL = -1, TDR_ENOMEM = -2, TDR_ECUDA = -3, TDR_ECAPACITY = -4, TDR_ELOST = -5,
        TDR_EOVERFLOW = -6, TDR_ESTATE = -7 };
@@ -63,6 +64,17 @@ typedef struct tdr_geometry {
    * fixed-source runs only */
   int32_t implicit_capture;                  /* 0 = analog (weights identically 1) */
   double w_roulette, w_survive;              /* roulette below w_roulette; a survivor continues with w_survive */
+  /* general cells (readings C1-C6): a universe with univ_nrings[u] == -1 is a list of cells, each the
+   * intersection of up to TDR_MAX_CSURF half-spaces of surfaces given in the frame of the lattice cell (X = x - cx[ix],
+   * Y = y - cy[iy], Z = z); the particle's `ring` then holds its cell within the universe.  All HOST arrays, copied at init. */
+  int32_t n_surf;                            /* 0 = none */
+  const int32_t *surf_kind;                  /* n_surf: 0 plane aX + bY + cZ = d; 1 sphere centre (a,b,c) radius d; 2 z-cylinder axis (a,b) radius d */
+  const double *surf_coef;                   /* n_surf*4: a, b, c, d */
+  int32_t n_cell;
+  const int32_t *univ_cell0, *univ_ncell;    /* n_univ: first cell / number of cells (<= 255) of a general universe */
+  const int32_t *cell_nsurf;                 /* n_cell: 1..TDR_MAX_CSURF */
+  const int32_t *cell_surf;                  /* n_cell*TDR_MAX_CSURF: +(s+1) = the side f_s >= 0, -(s+1) = the side f_s < 0 */
+  const int32_t *cell_mat;                   /* n_cell */
 } tdr_geometry;
 
 typedef struct tdr_materials {

@@ -178,18 +178,18 @@ double orc_surf_dist(int kind, const double *co, double X, double Y, double Z, d
     d = (co[3] - ((co[0] * X + co[1] * Y) + co[2] * Z)) / den;
   } else {
     const double ox = X - co[0], oy = Y - co[1], oz = kind == 1 ? Z - co[2] : 0.0, wz = kind == 1 ? w : 0.0;
-    const double a = (u * u + v * v) + wz * wz;
-    if (a == 0.0) return INFINITY;
-    const double b = (ox * u + oy * v) + oz * wz;
-    const double c = ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3];
-    double disc = b * b - a * c;
+    const double qa = (u * u + v * v) + wz * wz;
+    if (qa == 0.0) return INFINITY;
+    const double qb = (ox * u + oy * v) + oz * wz;
+    const double qc = ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3];
+    double disc = qb * qb - qa * qc;
     if (negative_side) {
       if (disc < 0.0) disc = 0.0;
-      d = (-b + sqrt(disc)) / a;
+      d = (-qb + sqrt(disc)) / qa;
     } else {
-      if (b >= 0.0) return INFINITY;
+      if (qb >= 0.0) return INFINITY;
       if (disc <= 0.0) return INFINITY;
-      d = (-b - sqrt(disc)) / a;
+      d = (-qb - sqrt(disc)) / qa;
     }
   }
   if (d < 0.0) d = 0.0;

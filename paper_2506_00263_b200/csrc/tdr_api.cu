@@ -129,8 +129,24 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
     for (int k = 0; k < ln[a]; k++) if (!(lp[a][k] < lp[a][k + 1])) return fail(TDR_EINVAL, "lattice planes of axis %d are not strictly ascending", a);
     for (int k = 0; k < g->mesh_n[a]; k++) if (!(mp[a][k] < mp[a][k + 1])) return fail(TDR_EINVAL, "mesh planes of axis %d are not strictly ascending", a);
   }
+  if (g->n_surf < 0 || g->n_surf > 32767) return fail(TDR_EINVAL, "bad surface count");
+  if (g->n_surf > 0) {                          // general cells: every index the device follows is checked here
+    if (!g->surf_kind || !g->surf_coef || !g->univ_cell0 || !g->univ_ncell || !g->cell_nsurf || !g->cell_surf || !g->cell_mat || g->n_cell < 1)
+      return fail(TDR_EINVAL, "general cells: null table");
+    for (int k = 0; k < g->n_surf; k++)
+      if (g->surf_kind[k] < 0 || g->surf_kind[k] > 2 || (g->surf_kind[k] > 0 && !(g->surf_coef[4 * k + 3] > 0.0))) return fail(TDR_EINVAL, "surface %d: bad kind or radius", k);
+    for (int k = 0; k < g->n_cell; k++) {
+      if (g->cell_nsurf[k] < 1 || g->cell_nsurf[k] > TDR_MAX_CSURF) return fail(TDR_EINVAL, "cell %d: 1..%d surfaces", k, TDR_MAX_CSURF);
+      if (g->cell_mat[k] < 0 || g->cell_mat[k] >= m->n_mat) return fail(TDR_EINVAL, "cell %d names material %d of %d", k, g->cell_mat[k], m->n_mat);
+      for (int j = 0; j < g->cell_nsurf[k]; j++) { const int r = g->cell_surf[k * TDR_MAX_CSURF + j]; if (r == 0 || abs(r) > g->n_surf) return fail(TDR_EINVAL, "cell %d names surface %d of %d", k, r, g->n_surf); }
+    }
+  }
   for (int u = 0; u < g->n_univ; u++) {
     const int nr = g->univ_nrings[u];
+    if (nr == -1 && g->n_surf > 0) {
+      if (g->univ_cell0[u] < 0 || g->univ_ncell[u] < 1 || g->univ_ncell[u] > 255 || g->univ_cell0[u] + g->univ_ncell[u] > g->n_cell) return fail(TDR_EINVAL, "universe %d: bad cell range", u);
+      continue;
+    }
     if (nr < 0 || nr > TDR_MAX_RINGS) return fail(TDR_EINVAL, "bad ring count");
     for (int r = 0; r < nr; r++) {
       const double R = g->univ_radius[u * TDR_MAX_RINGS + r];
@@ -189,6 +205,12 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
   UP(g->univ_nrings, g->n_univ, D.univ_nr); UP(g->univ_radius, g->n_univ * TDR_MAX_RINGS, D.univ_rad);
   UP(g->univ_mat, g->n_univ * (TDR_MAX_RINGS + 1), D.univ_mat);
   for (int a = 0; a < 3; a++) UP(mp[a], g->mesh_n[a] + 1, D.mesh[a]);
+  D.n_surf = g->n_surf; D.n_cell = g->n_surf > 0 ? g->n_cell : 0;
+  if (g->n_surf > 0) {
+    UP(g->surf_kind, g->n_surf, D.surf_kind); UP(g->surf_coef, 4 * g->n_surf, D.surf_coef);
+    UP(g->univ_cell0, g->n_univ, D.univ_cell0); UP(g->univ_ncell, g->n_univ, D.univ_ncell);
+    UP(g->cell_nsurf, g->n_cell, D.cell_nsurf); UP(g->cell_surf, g->n_cell * TDR_MAX_CSURF, D.cell_surf); UP(g->cell_mat, g->n_cell, D.cell_mat);
+  }
   D.n_t = g->n_tbins; D.implicit = g->implicit_capture != 0; D.w_roulette = g->w_roulette; D.w_survive = g->w_survive;
   if (D.n_t > 0) { UP(g->t_edges, D.n_t + 1, D.t_edges); if (m->G > 0) UP(m->speed, m->G, D.speed); }
   D.src_kind = g->src_kind; D.src_dir_kind = g->src_dir_kind; D.src_energy_kind = g->src_energy_kind; D.src_index = g->src_index;
@@ -568,7 +590,7 @@ static int run_async(tdr_problem *p, DevRun R) {
   if (!R.kmode) { k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull); LAUNCH_CHECK(); }   // the links of secondaries
   k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved, p->force_spill ? (1ull << 40) : 0ull);
   LAUNCH_CHECK();
-  const bool ext = p->dp.n_t > 0 || p->dp.implicit;           // the build with the time mesh / weights compiled in (ProbX)
+  const bool ext = p->dp.n_t > 0 || p->dp.implicit || p->dp.n_surf > 0;           // the build with the time mesh / weights compiled in (ProbX)
   if (ext) { if (p->split == 1) launch_async<CE, 1, true>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, true>(p, R, smem, threads); else launch_async<CE, 0, true>(p, R, smem, threads); }
   else { if (p->split == 1) launch_async<CE, 1, false>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, false>(p, R, smem, threads); else launch_async<CE, 0, false>(p, R, smem, threads); }
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
@@ -674,10 +696,10 @@ static int run_generation(tdr_problem *p, DevRun &R) {
   R.src_next = p->ctr + C_SRC_NEXT; R.sec_tail = p->ctr + C_SEC_TAIL; R.sec_head = p->ctr + C_SEC_HEAD;
   R.bank_count = p->ctr + C_BANK; R.hist_count = p->ctr + C_HIST;
   R.sec = p->sec; R.sec_time = p->sec_time; R.sec_w = p->sec_w; R.sec_cap = p->sec_cap; R.sec_limit = 0; R.sec_head0 = 0;
-  R.bank = p->bank; R.bank_cap = p->bank_cap;
+  R.bank = p->bank; R.bank_cap = p->bank_cap; R.err = p->out.err;
   R.hist_id = p->hist_id; R.hist_nseg = p->hist_nseg; R.hist_ncoll = p->hist_ncoll;
   if (p->scheme == 0) {
-    const bool ext = p->dp.n_t > 0 || p->dp.implicit;
+    const bool ext = p->dp.n_t > 0 || p->dp.implicit || p->dp.n_surf > 0;
     int rc = p->ce ? (ext ? run_stack<true, true>(p, R) : run_stack<true, false>(p, R)) : (ext ? run_stack<false, true>(p, R) : run_stack<false, false>(p, R));
     return rc ? rc : overflow_check(p);
   }
@@ -695,8 +717,9 @@ static int overflow_check(tdr_problem *p) {
 static int run_async_any(tdr_problem *p, DevRun &R) {
   // auto: the shared particle stash where the path is instruction bound (multigroup); the index stash where it is bound by
   // cross-section gathers and wants the L1 that a particle stash would take (continuous energy) — DESIGN.md section 6
-  if ((p->dp.n_t > 0 || p->dp.implicit) && p->stash > 0) return fail(TDR_EINVAL, "time-dependent and implicit-capture runs use the index stash (stash = auto|index)");
-  const int stash = p->stash >= 0 ? p->stash : ((p->ce || p->dp.n_t > 0 || p->dp.implicit) ? 0 : 2);
+  const bool ext = p->dp.n_t > 0 || p->dp.implicit || p->dp.n_surf > 0;
+  if (ext && p->stash > 0) return fail(TDR_EINVAL, "time-dependent, implicit-capture and general-cell runs use the index stash (stash = auto|index)");
+  const int stash = p->stash >= 0 ? p->stash : ((p->ce || ext) ? 0 : 2);
   if (stash == 2 && p->split != 1) return p->ce ? run_cstash<true>(p, R) : run_cstash<false>(p, R);
   if (stash == 1 && p->split != 1) return p->ce ? run_pstash<true>(p, R) : run_pstash<false>(p, R);
   return p->ce ? run_async<true>(p, R) : run_async<false>(p, R);      // index stash; the five-event decomposition always

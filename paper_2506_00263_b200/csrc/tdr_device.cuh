@@ -34,6 +34,8 @@ struct DevProb {
   const double *A, *nuc_nu, *wa, *wb;
   const u32 *hash; u32 hash_bmin, hash_n;    // X3: bucket -> first candidate grid index
   double grid_lo, grid_hi;
+  // general cells (readings C1-C6): a universe with univ_nr == -1 is a list of cells, each an intersection of half-spaces
+  int n_surf, n_cell; const int *surf_kind, *univ_cell0, *univ_ncell, *cell_nsurf, *cell_surf, *cell_mat; const double *surf_coef;
   u64 n_bins;
   static constexpr bool EXT = true;            // as a plain DevProb every extension is decided at run time (see ProbX)
 };
@@ -71,6 +73,7 @@ struct DevRun {
   u64 *outstanding, *slot_next, *starved; u64 W;
   u64 id_offset;                              // first source id of this run (multi-GPU sharding of a fixed source)
   int defer_death;                            // deaths are booked by the SOURCE event (asynchronous scheme)
+  int *err;                                   // the run's sticky error word (for the events that have no DevOut at hand)
 };
 
 struct Part {
@@ -241,6 +244,63 @@ __device__ __forceinline__ double dist_cyl(double X, double Y, double u, double 
   return d;
 }
 
+// ---------------------------------------------------------------------------------- C2-C4 general cells
+__device__ __forceinline__ double surf_eval(int kind, const double *co, double X, double Y, double Z) {   // C2: negative inside
+  if (kind == 0) return ((co[0] * X + co[1] * Y) + co[2] * Z) - co[3];
+  const double ox = X - co[0], oy = Y - co[1];
+  if (kind == 1) { const double oz = Z - co[2]; return ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3]; }
+  return (ox * ox + oy * oy) - co[3] * co[3];
+}
+
+// C3: distance to the surface for a particle known (from its cell) to be on the given side
+__device__ __forceinline__ double surf_dist(int kind, const double *co, double X, double Y, double Z, double u, double v, double w, bool negative_side) {
+  double d;
+  if (kind == 0) {
+    const double den = (co[0] * u + co[1] * v) + co[2] * w;
+    if (negative_side ? !(den > 0.0) : !(den < 0.0)) return TDR_INF;
+    d = (co[3] - ((co[0] * X + co[1] * Y) + co[2] * Z)) / den;
+  } else {
+    const double ox = X - co[0], oy = Y - co[1], oz = kind == 1 ? Z - co[2] : 0.0, wz = kind == 1 ? w : 0.0;
+    const double a = (u * u + v * v) + wz * wz;
+    if (a == 0.0) return TDR_INF;
+    const double b = (ox * u + oy * v) + oz * wz;
+    const double c = ((ox * ox + oy * oy) + oz * oz) - co[3] * co[3];
+    double disc = b * b - a * c;
+    if (negative_side) {
+      if (disc < 0.0) disc = 0.0;
+      d = (-b + sqrt(disc)) / a;
+    } else {
+      if (b >= 0.0) return TDR_INF;
+      if (disc <= 0.0) return TDR_INF;
+      d = (-b - sqrt(disc)) / a;
+    }
+  }
+  if (d < 0.0) d = 0.0;
+  return d;
+}
+
+// C4: the first cell of the universe all of whose half-spaces hold the point; a surface flagged in `crossed` (bit j = slot j
+// of cell `from`) is taken to be on the side opposite to the one `from` names.  -1: no such cell.
+__device__ __forceinline__ int locate_cell(const DevProb &P, int univ, double X, double Y, double Z, int from, u32 crossed) {
+  const int c0 = P.univ_cell0[univ], nc = P.univ_ncell[univ];
+  for (int k = 0; k < nc; k++) {
+    const int cell = c0 + k; bool ok = true;
+    for (int j = 0; j < P.cell_nsurf[cell] && ok; j++) {
+      const int r = P.cell_surf[cell * TDR_MAX_CSURF + j], sf = abs(r) - 1; const bool want_neg = r < 0;
+      int neg = -1;
+      if (from >= 0)
+        for (int i = 0; i < P.cell_nsurf[from]; i++) {
+          const int rf = P.cell_surf[from * TDR_MAX_CSURF + i];
+          if ((crossed >> i & 1u) && abs(rf) - 1 == sf) neg = !(rf < 0);
+        }
+      if (neg < 0) neg = surf_eval(P.surf_kind[sf], P.surf_coef + 4 * sf, X, Y, Z) < 0.0;
+      ok = (neg != 0) == want_neg;
+    }
+    if (ok) return k;
+  }
+  return -1;
+}
+
 __device__ __forceinline__ int find_bin(const double *pl, int n, double x) {   // G2
   int k = 0;
 #pragma unroll 1
@@ -253,6 +313,11 @@ __device__ __forceinline__ int locate_ring(const DevProb &P, int univ, double X,
   double r2 = X * X + Y * Y;
   for (int r = 0; r < nr; r++) { double R = P.univ_rad[univ * TDR_MAX_RINGS + r]; if (r2 < R * R) return r; }
   return nr;
+}
+
+__device__ __forceinline__ int locate_in_universe(const DevProb &P, int univ, double X, double Y, double Z) {   // G2 / C4
+  if (P.univ_nr[univ] < 0) return locate_cell(P, univ, X, Y, Z, -1, 0u);
+  return locate_ring(P, univ, X, Y);
 }
 
 __device__ __forceinline__ int sample_cdf(const double *cdf, int n, double xi) {   // X1

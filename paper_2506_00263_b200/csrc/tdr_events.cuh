@@ -5,7 +5,8 @@
 #include "tdr_device.cuh"
 
 // flags produced by MOVE
-enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512, F_TIME = 1024 };
+enum { F_COLLIDE = 1, F_DX = 2, F_DY = 4, F_DZ = 8, F_DOUT = 16, F_DIN = 32, F_MX = 64, F_MY = 128, F_MZ = 256, F_LOST = 512, F_TIME = 1024,
+       F_CS0 = 2048 /* .. F_CS0 << 5: surface slot j of the current general cell was reached */ };
 
 // per-block accumulators in shared memory, flushed once per kernel (finalize hook).  Every 64-bit sum
 // is two 32-bit words updated with native shared atomics: the carry out of the low word goes to the high word, so
@@ -91,8 +92,10 @@ __device__ __forceinline__ void tally_add(u64 *arr, u32 *lo, u32 *hi, bool priv,
 }
 
 // ---------------------------------------------------------------------------------- helpers
-__device__ __forceinline__ int cell_material(const DevProb &P, const Part &p, int &univ) {
+template <class PT>
+__device__ __forceinline__ int cell_material(const PT &P, const Part &p, int &univ) {
   univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
+  if (PT::EXT && P.n_surf > 0 && P.univ_nr[univ] < 0) return P.cell_mat[P.univ_cell0[univ] + p.ring];
   return P.univ_mat[univ * (TDR_MAX_RINGS + 1) + p.ring];
 }
 
@@ -109,8 +112,8 @@ __device__ __forceinline__ int grid_index(const DevProb &P, double El) {   // X3
 }
 
 // ---------------------------------------------------------------------------------- T1 LOOKUP
-template <bool CE>
-__device__ __forceinline__ void ev_lookup(const DevProb &P, const double *mg, const Part &p, double &St, double &nsf,
+template <bool CE, class PT>
+__device__ __forceinline__ void ev_lookup(const PT &P, const double *mg, const Part &p, double &St, double &nsf,
                                           int &gi, double &f) {
   int univ; int mat = cell_material(P, p, univ);
   if (!CE) {
@@ -156,6 +159,16 @@ __device__ __forceinline__ void ev_move(const PT &P, u64 seed, u32 gen, Part &p,
     if (out1) dout = d1; else din = d1;
     if (out1 && p.ring > 0) din = dist_cyl(X, Y, p.u, p.v, P.univ_rad[univ * TDR_MAX_RINGS + p.ring - 1], false);
   }
+  double dcs[TDR_MAX_CSURF]; int ncs = 0;                             // C5: the surfaces of the current general cell
+  if (PT::EXT && nr < 0) {
+    const int gcell = P.univ_cell0[univ] + p.ring; ncs = P.cell_nsurf[gcell];
+    const double X = p.x - P.cx[p.ix], Y = p.y - P.cy[p.iy];
+#pragma unroll
+    for (int j = 0; j < TDR_MAX_CSURF; j++) {
+      dcs[j] = TDR_INF;
+      if (j < ncs) { const int r = P.cell_surf[gcell * TDR_MAX_CSURF + j], sf = abs(r) - 1; dcs[j] = surf_dist(P.surf_kind[sf], P.surf_coef + 4 * sf, X, Y, p.z, p.u, p.v, p.w, r < 0); }
+    }
+  }
   // mesh planes: a mesh cell bounded by the very same plane values as the lattice cell gives the very same quotient
   const double mxl = P.mesh[0][p.mx], mxh = P.mesh[0][p.mx + 1], myl = P.mesh[1][p.my], myh = P.mesh[1][p.my + 1];
   const double mzl = P.mesh[2][p.mz], mzh = P.mesh[2][p.mz + 1];
@@ -172,6 +185,10 @@ __device__ __forceinline__ void ev_move(const PT &P, u64 seed, u32 gen, Part &p,
   if (dz < ds) ds = dz;
   if (dout < ds) ds = dout;
   if (din < ds) ds = din;
+  if (PT::EXT && ncs > 0) {
+#pragma unroll
+    for (int j = 0; j < TDR_MAX_CSURF; j++) if (dcs[j] < ds) ds = dcs[j];
+  }
   if (dmx < ds) ds = dmx;
   if (dmy < ds) ds = dmy;
   if (dmz < ds) ds = dmz;
@@ -183,6 +200,10 @@ __device__ __forceinline__ void ev_move(const PT &P, u64 seed, u32 gen, Part &p,
   if (collide) flags = F_COLLIDE;
   else flags = (dx == d ? F_DX : 0) | (dy == d ? F_DY : 0) | (dz == d ? F_DZ : 0) | (dout == d ? F_DOUT : 0) |
                (din == d ? F_DIN : 0) | (dmx == d ? F_MX : 0) | (dmy == d ? F_MY : 0) | (dmz == d ? F_MZ : 0) | ((PT::EXT && dtm == d) ? F_TIME : 0);
+  if (PT::EXT && ncs > 0 && !collide) {
+#pragma unroll
+    for (int j = 0; j < TDR_MAX_CSURF; j++) if (j < ncs && dcs[j] == d) flags |= F_CS0 << j;
+  }
   p.x = p.x + d * p.u; p.y = p.y + d * p.v; p.z = p.z + d * p.w;       // G6
   if (PT::EXT && P.n_t > 0) p.t = p.t + d / vel;                                  // TD3
 }
@@ -350,8 +371,13 @@ __device__ __forceinline__ bool ev_surface(const PT &P, const DevRun &R, BlockAc
   if (flags & F_DIN) p.ring -= 1;
   if (moved_xy || moved_z) {
     int nu2 = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
-    if (moved_xy) p.ring = P.univ_nr[nu2];
+    if (PT::EXT && P.n_surf > 0 && P.univ_nr[nu2] < 0) { if (moved_xy || nu2 != univ) p.ring = locate_in_universe(P, nu2, p.x - P.cx[p.ix], p.y - P.cy[p.iy], p.z); }
+    else if (moved_xy) p.ring = P.univ_nr[nu2];
     else if (nu2 != univ) p.ring = locate_ring(P, nu2, p.x - P.cx[p.ix], p.y - P.cy[p.iy]);
+    if (PT::EXT && p.ring < 0) { atomicExch(R.err, TDR_ELOST); p.ring = 0; }
+  } else if (PT::EXT && (flags >> 11 & 63u)) {                         // C6: through one or more surfaces of a general cell
+    p.ring = locate_cell(P, univ, p.x - P.cx[p.ix], p.y - P.cy[p.iy], p.z, P.univ_cell0[univ] + p.ring, flags >> 11 & 63u);
+    if (p.ring < 0) { atomicExch(R.err, TDR_ELOST); p.ring = 0; }
   }
   for (u32 mf = flags & (F_MX | F_MY | F_MZ); mf; mf &= mf - 1) {      // mesh planes, the same way (indices clamp at the mesh box)
     const int a = (mf & F_MX) ? 0 : (mf & F_MY) ? 1 : 2;
@@ -400,7 +426,8 @@ __device__ TDR_COLD void birth_primary(const DevProb &P, const double *mg, const
   p.ix = find_bin(P.xp, P.nx, p.x); p.iy = find_bin(P.yp, P.ny, p.y); p.iz = find_bin(P.zp, P.nz, p.z);
   p.mx = find_bin(P.mesh[0], P.mesh_n[0], p.x); p.my = find_bin(P.mesh[1], P.mesh_n[1], p.y); p.mz = find_bin(P.mesh[2], P.mesh_n[2], p.z);
   int univ = P.cell_univ[((size_t)p.iz * P.ny + p.iy) * P.nx + p.ix];
-  p.ring = locate_ring(P, univ, p.x - P.cx[p.ix], p.y - P.cy[p.iy]);
+  p.ring = locate_in_universe(P, univ, p.x - P.cx[p.ix], p.y - P.cy[p.iy], p.z);
+  if (p.ring < 0) { atomicExch(R.err, TDR_ELOST); p.ring = 0; }
   birth_common<CE>(P, mg, R, acc, p, 0, false);
 }
 

@@ -29,7 +29,9 @@ class tdr_geometry(C.Structure):
                 ("src_dir_kind", C.c_int32), ("src_dir", C.c_double * 3),
                 ("src_energy_kind", C.c_int32), ("src_index", C.c_int32), ("src_energy", C.c_double),
                 ("tally_scale_log2", C.c_int32), ("n_tbins", C.c_int32), ("t_edges", PD),
-                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double)]
+                ("implicit_capture", C.c_int32), ("w_roulette", C.c_double), ("w_survive", C.c_double),
+                ("n_surf", C.c_int32), ("surf_kind", PI), ("surf_coef", PD), ("n_cell", C.c_int32), ("univ_cell0", PI), ("univ_ncell", PI),
+                ("cell_nsurf", PI), ("cell_surf", PI), ("cell_mat", PI)]
 
 
 class tdr_materials(C.Structure):

@@ -195,6 +195,12 @@ def two_region(kind="pin", n=200000, seed=1):
         geo = geometry([-h, h], [-h, h], [-INF, INF], [0], [((R1, R), (1, 0, 1))], [1, 1, 1, 1, 0, 0],
                        src_kind=1, src_lo=(-h, -h, 0.0), src_hi=(h, h, 0.0))
         frac = pi * (R * R - R1 * R1) / (4 * h * h)
+    elif kind == "strips":
+        # two lattice cells of the SAME universe of general cells, split by the plane X = 0.2 of the cell frame: a particle that
+        # goes through the lattice plane leaves the moderator strip of one cell and enters the fuel strip of the next
+        geo = geometry([-1.0, 0.0, 1.0], [-1.0, 1.0], [-1.0, 1.0], [0, 0], [("cells", [((-1,), 0), ((+1,), 1)])], [1] * 6,
+                       src_kind=1, src_lo=(-1.0, -1.0, -1.0), src_hi=(1.0, 1.0, 1.0), surfaces=[("plane", 1.0, 0.0, 0.0, 0.2)])
+        frac = 0.7
     elif kind in ("sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells"):
         # general cells (readings C1-C6): "fuel" (material 0) is a cell, or several, of a universe of general cells
         c = 1.0                                                # half width of the cube; z is finite here (spheres)
@@ -347,6 +353,29 @@ def cfg1(n=1000000, n_inactive=20, n_active=50, seed=1, identical_materials=Fals
         for k in ("sig_t", "sig_s", "sig_f", "nu", "chi"):
             mats[k][1] = mats[k][0]
     return Problem("cfg1", geo, mats, None, "k", n, n_inactive, n_active, seed)
+
+
+def general_cells(mode="k", n=40003, n_inactive=1, n_active=2, seed=1, n_ebins=None):
+    """Universes of general cells (readings C1-C6) in a k-eigenvalue or fixed-source run: a 2 x 2 x 2 lattice with
+    vacuum on +x, +z and reflection elsewhere; universe 0 = a fuel sphere cut by an oblique plane (two fuel cells) inside
+    moderator, universe 1 = cfg1's ring pin, universe 2 = a fuel lens (two spheres) beside an off-axis guide cylinder.
+    7-group materials of cfg1; with n_ebins the continuous-energy pin cell of cfg3 / cfg4 in the same geometry."""
+    surf = [("sphere", 0.05, -0.04, 0.0, 0.5), ("plane", 1.0, 1.0, 2.0, 0.1),                   # universe 0
+            ("sphere", -0.15, 0.0, 0.1, 0.42), ("sphere", 0.15, 0.0, 0.1, 0.42), ("zcyl", 0.0, 0.52, 0.0, 0.08)]   # universe 2
+    u0 = ("cells", [((-1, -2), 0), ((-1, +2), 0), ((+1,), 1)])
+    u2 = ("cells", [((-3, -4), 0), ((-5,), 1), ((+3, +4, +5), 1), ((-3, +4), 1), ((+3, -4), 1)])
+    xp = [-0.63, 0.63, 1.89]; zp = [-0.6, 0.6, 1.8]
+    cu = [0, 1, 2, 0, 1, 2, 0, 1]
+    kw = dict(src_kind=1, src_lo=(xp[0], xp[0], zp[0]), src_hi=(xp[-1], xp[-1], zp[-1]), surfaces=surf, mesh=(xp, xp, [zp[0], zp[-1]]))
+    bc = [1, 0, 1, 1, 1, 0]
+    universes = [u0, ((0.54,), (0, 1)), u2]
+    if n_ebins is None:
+        geo = geometry(xp, xp, zp, cu, universes, bc, by_group=1, **kw)
+        return Problem("general_cells_" + mode, geo, _mg_set(["fuel", "mod"]), None, mode, n, n_inactive if mode == "k" else 0, n_active if mode == "k" else 0, seed)
+    base = cfg4(n=n, n_inactive=n_inactive, n_active=n_active, seed=seed, n_ebins=n_ebins) if mode == "k" else cfg3(n=n, n_ebins=n_ebins, seed=seed)
+    g0 = base.geometry
+    geo = geometry(xp, xp, zp, cu, universes, bc, e_edges=g0["e_edges"], src_energy=("watt", 2) if mode == "k" else ("mono", 14.0e6), **kw)
+    return Problem("general_cells_ce_" + mode, geo, base.materials, base.xs, mode, n, base.n_inactive, base.n_active, seed)
 
 
 def cfg2(n=10000000, n_inactive=6, n_active=18, seed=1):

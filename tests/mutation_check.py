@@ -19,6 +19,17 @@ PINS = ["tests/test_oracle_pins.py", "tests/test_oracle_pins_transport.py"]
 
 # (name, text in orc.c, replacement, what it breaks)
 MUTANTS = [
+    ("csg_plane_side", "if (negative_side ? !(den > 0.0) : !(den < 0.0)) return INFINITY;", "if (negative_side ? !(den < 0.0) : !(den > 0.0)) return INFINITY;", "C3 plane reachable from the wrong side"),
+    ("csg_inside_root", "d = (-qb + sqrt(disc)) / qa;", "d = (-qb - sqrt(disc)) / qa;", "C3 leaving root of a sphere / cylinder"),
+    ("csg_outside_root", "d = (-qb - sqrt(disc)) / qa;", "d = (-qb + sqrt(disc)) / qa;", "C3 entering root of a sphere / cylinder"),
+    ("csg_sphere_z", "oz = kind == 1 ? Z - co[2] : 0.0", "oz = kind == 1 ? Z + co[2] : 0.0", "C3 sphere centre z"),
+    ("csg_eval_plane", "if (kind == 0) return ((co[0] * X + co[1] * Y) + co[2] * Z) - co[3];", "if (kind == 0) return ((co[0] * X + co[1] * Y) + co[2] * Z) + co[3];", "C2 plane function"),
+    ("csg_eval_cyl", "return (ox * ox + oy * oy) - co[3] * co[3];", "return (ox * ox + oy * oy) - co[3];", "C2 cylinder function"),
+    ("csg_crossed_side", "if ((crossed >> i & 1u) && abs(rf) - 1 == sf) neg = !(rf < 0);", "if ((crossed >> i & 1u) && abs(rf) - 1 == sf) neg = (rf < 0);", "C4 a crossed surface keeps its old side"),
+    ("csg_tie_first_only", "for (int j = 0; j < ncs; j++) if (dcs[j] == d) crossed |= 1u << j;", "for (int j = 0; j < ncs; j++) if (dcs[j] == d) { crossed |= 1u << j; break; }", "C6 only the first of several surfaces met at once is crossed (EQUIVALENT in practice: ties have measure zero)"),
+    ("csg_candidate", "for (int j = 0; j < ncs; j++) if (dcs[j] < ds) ds = dcs[j];", "for (int j = 1; j < ncs; j++) if (dcs[j] < ds) ds = dcs[j];", "C5 the cell's first surface is not a candidate"),
+    ("csg_relocate_xy", "{ if (moved_xy || nu2 != univ) q->ring = locate_in_universe(", "{ if (nu2 != univ) q->ring = locate_in_universe(", "C6 no re-location at a lattice plane between cells of the same general universe"),
+    ("csg_material", "return p->cell_mat[p->univ_cell0[univ] + ring];", "return p->cell_mat[ring];", "C1 material of a cell: universe offset dropped"),
     ("rot_swap_uv", "un = mul * u + k * ((u * w) * cphi - v * sphi);", "un = mul * u + k * ((v * w) * cphi - u * sphi);", "T6 rotation: u/v swapped in the first component"),
     ("rot_sign_vn", "vn = mul * v + k * ((v * w) * cphi + u * sphi);", "vn = mul * v + k * ((v * w) * cphi - u * sphi);", "T6 rotation: sign of the sin(phi) term of v'"),
     ("rot_sign_wn", "wn = mul * w - (k * ow) * cphi;", "wn = mul * w + (k * ow) * cphi;", "T6 rotation: sign of the w' correction"),

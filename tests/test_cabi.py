@@ -88,6 +88,13 @@ def test_init_rejects_out_of_range_tables_with_einval():
     assert broken(mk3, lambda p: p.geometry["e_edges"].__setitem__(2, 0.0)) == EINVAL
     mk4 = lambda: W.cfg4(n=10, n_grid=500)
     assert broken(mk4, lambda p: p.geometry.__setitem__("src_index", 3)) == EINVAL                   # Watt nuclide out of range
+    mk5 = lambda: W.general_cells("k", n=10)                                                          # general cells (readings C1-C6)
+    assert broken(mk5, lambda p: p.geometry["cell_surf"].__setitem__((0, 0), 9)) == EINVAL           # surface out of range
+    assert broken(mk5, lambda p: p.geometry["cell_surf"].__setitem__((1, 1), 0)) == EINVAL           # a cell naming no surface
+    assert broken(mk5, lambda p: p.geometry["cell_mat"].__setitem__(2, 5)) == EINVAL
+    assert broken(mk5, lambda p: p.geometry["surf_kind"].__setitem__(0, 3)) == EINVAL
+    assert broken(mk5, lambda p: p.geometry["surf_coef"].__setitem__((0, 3), -0.5)) == EINVAL        # negative radius
+    assert broken(mk5, lambda p: p.geometry["univ_ncell"].__setitem__(2, 9)) == EINVAL               # cells beyond the table
     # untouched problems pass validation (the return code is then 0 on a GPU box, TDR_ECUDA = -3 without a device)
-    for mk in (mk2, mk3, mk4, W.cfg0, lambda: W.cfg1(n=10), lambda: W.slab(1.0, 2.0, n=10), lambda: W.ce_slowing_down(n=10)):
+    for mk in (mk2, mk3, mk4, mk5, W.cfg0, lambda: W.cfg1(n=10), lambda: W.slab(1.0, 2.0, n=10), lambda: W.ce_slowing_down(n=10)):
         assert _init_rc(mk()) in (0, -3)

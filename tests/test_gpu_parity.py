@@ -364,3 +364,39 @@ def test_implicit_capture_and_roulette_parity(scheme, decomp):
         assert g["totals"]["n_roulette"] > 0 and g["totals"]["n_abs"] == 0
     o, g, _ = run_both(ic(W.cfg3(n=5003, n_ebins=1)), scheme=scheme, decomposition=decomp, window=1024)
     assert_same(o, g, "cfg3_ic/window=1024")
+
+
+# ------------------------------------------------------------------ universes of general cells (readings C1-C6)
+@pytest.mark.parametrize("scheme,decomp", SCHEMES)
+def test_general_cells_parity(scheme, decomp):
+    """Planes, spheres and off-axis cylinders as cell boundaries, beside a ring universe in one lattice: k-eigenvalue and fixed
+    source, multigroup and continuous energy, plus two of the volume-pin geometries (the lens: two surfaces met at once)."""
+    for p in (W.general_cells("k"), W.general_cells("fixed", n=20011), W.general_cells("k", n=20011, n_ebins=100),
+              W.general_cells("fixed", n=5003, n_ebins=100), W.two_region("lens", n=30011), W.two_region("shell", n=30011)):
+        o, g, d = run_both(p, scheme=scheme, decomposition=decomp)
+        assert_same(o, g, f"{p.name}/{scheme}/{decomp}")
+        assert g["totals"]["n_cross"] > 0
+
+
+def test_general_cells_full_generation_and_refusals():
+    from paper_2506_00263_b200 import tdr
+    p = W.general_cells("k", n=1000003, n_inactive=1, n_active=1)
+    for scheme in ("async", "stack"):
+        o, g, _ = run_both(p, scheme=scheme)
+        assert_same(o, g, f"general cells at 1e6/{scheme}")
+    P = tdr.Problem(W.general_cells("k", n=1000), scheme="async", stash="shared")     # the particle stashes are built without them
+    with pytest.raises(tdr.TdrError) as e:
+        P.run()
+    assert e.value.code == -1
+    P.close()
+    # a cell list that does not cover space: a particle that finds no cell is TDR_ELOST on both sides
+    bad = W.two_region("sphere", n=2000)
+    bad.geometry["cell_surf"][1, 0] = -1                       # both cells now name the inside of the sphere
+    P = tdr.Problem(bad)
+    with pytest.raises(tdr.TdrError) as e:
+        P.run()
+    assert e.value.code == -5
+    P.close()
+    from oracle import orc
+    with pytest.raises(RuntimeError, match="-5"):
+        orc.run(bad)
