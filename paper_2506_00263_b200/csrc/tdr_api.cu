@@ -361,12 +361,17 @@ int tdr_bind_workspace(tdr_problem *p, void *ptr, uint64_t bytes, void *stream) 
 }
 
 // ---------------------------------------------------------------------------------- launch helpers
+// grid = SMs x resident CTAs; 0 when the kernel cannot be launched with this much dynamic shared memory (the callers turn that
+// into TDR_EINVAL).  Above the default 48 KB the kernel is opted in to large shared memory first.
 template <class K>
 static int grid_for(tdr_problem *p, K kernel, size_t smem, int threads = 256) {
-  int bps = p->blocks_per_sm;
-  if (bps <= 0) { if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kernel, threads, smem) != cudaSuccess || bps < 1) bps = 1; }
+  if (smem > 48 * 1024 && cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+  int occ = 0;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, smem) != cudaSuccess || occ < 1) { cudaGetLastError(); return 0; }
+  const int bps = p->blocks_per_sm > 0 ? p->blocks_per_sm : occ;
   return p->num_sms * bps;
 }
+#define GRID_OR_FAIL(g, what) do { if ((g) < 1) return fail(TDR_EINVAL, "%s: the kernel does not fit an SM with %zu bytes of dynamic shared memory (smaller multigroup table, fewer tally bins below 257, fewer stash_links or threads)", what, smem); } while (0)
 
 struct KTimer {                                   // optional CUDA-event bracket around the dominant kernel's launches
   tdr_problem *p; bool on;
@@ -464,6 +469,7 @@ static int build_stack_graph(tdr_problem *p, size_t smem) {
   CK(cudaGraphAddNode(&node, p->sg_graph, nullptr, 0, &np));
   cudaGraph_t body = np.conditional.phGraph_out[0];
   StackGrids G; stack_grids<CE, true, EXT>(p, smem, G);
+  GRID_OR_FAIL(p->split == 1 ? G.ev[EV_MOVE] : G.step, "stack scheme");
   DevRun none; memset(&none, 0, sizeof none);
   CK(cudaStreamBeginCaptureToGraph(p->sg_capture, body, nullptr, nullptr, 0, cudaStreamCaptureModeRelaxed));
   const int per_pass = remap_iteration<CE, true, EXT>(p, none, p->sg_capture, smem, G, 0, 1 << 30);
@@ -490,6 +496,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
   const size_t smem = smem_bytes(p);
   u64 *ctr = p->ctr; u64 *h = p->h_ctr;
   const int g_src = grid_for(p, k_source<CE>, smem);
+  GRID_OR_FAIL(g_src, "stack scheme");
   const u64 W = p->W;
   u64 h_src_next = 0, h_sec_tail = 0, h_sec_head = 0;
   auto source = [&](u32 *stack, u64 *count, u64 n_sec, u64 n) -> int {
@@ -509,7 +516,10 @@ static int run_stack(tdr_problem *p, DevRun R) {
   u64 n_in = n0;
   StackGrids G;
   if (dev) { if (!p->sg_exec && (rc = build_stack_graph<CE, EXT>(p, smem))) return rc; }
-  else stack_grids<CE, false, EXT>(p, smem, G);
+  else {
+    stack_grids<CE, false, EXT>(p, smem, G);
+    GRID_OR_FAIL(split ? G.ev[EV_MOVE] : G.step, "stack scheme");
+  }
   for (;;) {
     R.sec_limit = h_sec_tail; R.sec_head0 = h_sec_head;
     if (dev) {
@@ -549,6 +559,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
       // tail drain: the few particles left are followed to their death in ONE launch (k_drain).  Also under the five-event
       // decomposition: after a whole iteration every survivor waits on the LOOKUP stack, i.e. at the start of a segment.
       const int blocks = (int)((alive + 63) / 64);
+      if (smem > 48 * 1024) CK(cudaFuncSetAttribute(k_drain<CE, EXT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
       { KTimer td(p, true); k_drain<CE, EXT><<<blocks, 64, smem, st>>>(p->dp, p->out, R, p->soa, live_stack(it), live_count(it)); }
       LAUNCH_CHECK(); p->diag.kernel_launches++; p->diag.iterations++;
       CK(cudaMemcpyAsync(h, ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));
@@ -575,6 +586,7 @@ static int run_stack(tdr_problem *p, DevRun R) {
 template <bool CE, int MODE, bool EXT>
 static int launch_async(tdr_problem *p, const DevRun &R, size_t smem, int threads) {
   int grid = grid_for(p, k_async<CE, MODE, EXT>, smem, threads);
+  GRID_OR_FAIL(grid, "asynchronous scheme");
   KTimer t(p, true);
   k_async<CE, MODE, EXT><<<grid, threads, smem, p->stream>>>(p->dp, p->out, R, p->soa, p->am, p->pm, p->stash_links, (u64)p->idle_timeout_s * 1000000000ull,
                                                         (u32)p->slots_per_warp, p->lockstep, (u32)(p->seg_per_event ? p->seg_per_event : (CE ? 5 : 2)));
@@ -591,8 +603,10 @@ static int run_async(tdr_problem *p, DevRun R) {
   k_async_init<<<64, 256, 0, st>>>(p->am, R.outstanding, R.src_total, R.slot_next, R.starved, p->force_spill ? (1ull << 40) : 0ull);
   LAUNCH_CHECK();
   const bool ext = p->dp.n_t > 0 || p->dp.implicit || p->dp.n_surf > 0;           // the build with the time mesh / weights compiled in (ProbX)
-  if (ext) { if (p->split == 1) launch_async<CE, 1, true>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, true>(p, R, smem, threads); else launch_async<CE, 0, true>(p, R, smem, threads); }
-  else { if (p->split == 1) launch_async<CE, 1, false>(p, R, smem, threads); else if (p->split == 2) launch_async<CE, 2, false>(p, R, smem, threads); else launch_async<CE, 0, false>(p, R, smem, threads); }
+  int lrc;
+  if (ext) lrc = p->split == 1 ? launch_async<CE, 1, true>(p, R, smem, threads) : p->split == 2 ? launch_async<CE, 2, true>(p, R, smem, threads) : launch_async<CE, 0, true>(p, R, smem, threads);
+  else lrc = p->split == 1 ? launch_async<CE, 1, false>(p, R, smem, threads) : p->split == 2 ? launch_async<CE, 2, false>(p, R, smem, threads) : launch_async<CE, 0, false>(p, R, smem, threads);
+  if (lrc) return lrc;
   LAUNCH_CHECK(); p->diag.kernel_launches += 2; p->diag.iterations++;
   u64 *h = p->h_ctr;
   CK(cudaMemcpyAsync(h, p->ctr, C_COUNT * 8, cudaMemcpyDeviceToHost, st));

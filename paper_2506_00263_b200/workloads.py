@@ -201,6 +201,13 @@ def two_region(kind="pin", n=200000, seed=1):
         geo = geometry([-1.0, 0.0, 1.0], [-1.0, 1.0], [-1.0, 1.0], [0, 0], [("cells", [((-1,), 0), ((+1,), 1)])], [1] * 6,
                        src_kind=1, src_lo=(-1.0, -1.0, -1.0), src_hi=(1.0, 1.0, 1.0), surfaces=[("plane", 1.0, 0.0, 0.0, 0.2)])
         frac = 0.7
+    elif kind == "two_universes":
+        # two universes of general cells side by side whose cell lists name the materials in opposite order: fuel inside the
+        # sphere of the first, fuel OUTSIDE the (smaller) sphere of the second
+        surf = [("sphere", 0.0, 0.0, 0.0, 0.45), ("sphere", 0.1, 0.0, 0.0, 0.3)]
+        geo = geometry([-1.0, 0.0, 1.0], [-0.5, 0.5], [-0.5, 0.5], [0, 1], [("cells", [((-1,), 0), ((+1,), 1)]), ("cells", [((-2,), 1), ((+2,), 0)])],
+                       [1] * 6, src_kind=1, src_lo=(-1.0, -0.5, -0.5), src_hi=(1.0, 0.5, 0.5), surfaces=surf)
+        frac = (4.0 / 3.0 * pi * 0.45 ** 3 + (1.0 - 4.0 / 3.0 * pi * 0.3 ** 3)) / 2.0
     elif kind in ("sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells"):
         # general cells (readings C1-C6): "fuel" (material 0) is a cell, or several, of a universe of general cells
         c = 1.0                                                # half width of the cube; z is finite here (spheres)

@@ -214,7 +214,9 @@ def test_results_do_not_depend_on_the_launch_configuration():
     from paper_2506_00263_b200 import tdr
     for kw in (dict(scheme="stack", blocks_per_sm=1), dict(scheme="stack", blocks_per_sm=2), dict(scheme="stack", blocks_per_sm=4, window=50000),
                dict(scheme="async", async_threads=256), dict(scheme="async", async_threads=512, stash_links=16),
-               dict(scheme="async", async_threads=128, lockstep=0, slots_per_warp=64), dict(scheme="async", decomposition="split", async_threads=256)):
+               dict(scheme="async", async_threads=128, lockstep=0, slots_per_warp=64), dict(scheme="async", decomposition="split", async_threads=256),
+               dict(scheme="async", stash="index", stash_links=64),          # 148 KB of stash per CTA: opted in to large shared memory
+               dict(scheme="stack", device_loop=0), dict(scheme="stack", decomposition="hybrid", device_loop=0, sync_every=2)):
         P = tdr.Problem(p, **kw)
         g = P.run()
         P.close()

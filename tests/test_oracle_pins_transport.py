@@ -509,7 +509,7 @@ def _halfspace_fraction():
     return float(np.mean(xmax + 1) / 2)
 
 
-@pytest.mark.parametrize("kind", ["sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells", "strips"])
+@pytest.mark.parametrize("kind", ["sphere", "halfspace", "offcyl", "shell", "lens", "lattice_cells", "strips", "two_universes"])
 def test_general_cells_split_a_flat_flux_by_volume(kind):
     """The flat-flux volume pin on universes of general cells: a wrong root or side in the distance to a sphere, plane or
     cylinder, a cell search that ignores the crossed surface, a missed tie on the rim of the lens or a missed re-location at a
