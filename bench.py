@@ -303,7 +303,7 @@ class Runner:
             "segments_per_step": seg_step, "histories_per_step": hist_step,
             "e2e": {"value": seg_step * e2e_steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": bi, "d2h_bytes_per_step": bo, "steps": e2e_steps},
             "gpu_launches": int(launches), "digest": f"{res['totals']['digest']:016x}", "k_mean": res["k_mean"] if prob.mode == "k" else None,
-            "roofline": {"bound": "hbm", "achieved": ach, "peak": self.peak, "unit": "GB/s", "frac": ach / self.peak, "traffic": traffic,
+            "roofline": {"bound": "hbm", "kind": "modelled algorithmic bytes / measured kernel time (traffic = measured DRAM bytes)", "achieved": ach, "peak": self.peak, "unit": "GB/s", "frac": ach / self.peak, "traffic": traffic,
                          "peak_source": self.peak_src, "kernel": kname, "kernel_share_of_step": step_ms / ms if ms > 0 else None,
                          "avg_launch_us": 1e3 * step_ms / max(step_launches, 1),
                          "algorithmic_bytes_per_launch": alg_bytes * steps / max(step_launches, 1),

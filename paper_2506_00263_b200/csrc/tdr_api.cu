@@ -7,6 +7,7 @@
 #include <cstring>
 #include <string>
 #include <vector>
+#include <nvtx3/nvToolsExt.h>      // header-only NVTX 3: ranges around runs, generations and population control (no-ops without a tool)
 #include "tdr_stack.cuh"
 #include "tdr_split.cuh"
 #include "tdr_async.cuh"
@@ -15,6 +16,8 @@
 #include "tdr_peaks.cuh"
 
 static thread_local char g_err[512] = "";
+struct NvtxRange { explicit NvtxRange(const char *name) { nvtxRangePushA(name); } ~NvtxRange() { nvtxRangePop(); } };
+
 static int fail(int code, const char *fmt, ...) {
   va_list ap; va_start(ap, fmt); vsnprintf(g_err, sizeof g_err, fmt, ap); va_end(ap);
   return code;
@@ -704,6 +707,7 @@ static int run_async_any(tdr_problem *p, DevRun &R);
 
 // one generation (or the whole fixed-source run) under the selected scheme
 static int run_generation(tdr_problem *p, DevRun &R) {
+  NvtxRange nvtx(R.kmode ? "tdr generation" : "tdr fixed-source transport");
   cudaStream_t st = p->stream;
   CK(cudaMemsetAsync(p->ctr, 0, C_COUNT * 8, st));
   CK(cudaMemsetAsync(p->out.PPc, 0, 16, st));
@@ -817,6 +821,7 @@ int tdr_k_generation(tdr_problem *p, uint32_t gen, int active, double k_prev, in
 
 int tdr_k_population_control(tdr_problem *p, uint32_t gen_next, double pr, uint64_t *n_next) {
   if (!p || !n_next || !p->ws) return fail(TDR_EINVAL, "bad argument");
+  NvtxRange nvtx("tdr population control");
   RunClock clk(p->stream);
   cudaStream_t st = p->stream;
   const u64 M = p->k_last_bank;
@@ -883,6 +888,7 @@ int tdr_tally_sizes(const tdr_problem *p, tdr_sizes *o) {
 
 int tdr_read_tallies(const tdr_problem *p, tdr_tallies *t) {
   if (!p || !t) return fail(TDR_EINVAL, "null argument");
+  NvtxRange nvtx("tdr read_tallies");
   if (!p->ran) return fail(TDR_ESTATE, "no completed run");
   cudaStream_t st = p->stream;
   if (t->flux) CK(cudaMemcpyAsync(t->flux, p->out.flux, p->dp.n_bins * 8, cudaMemcpyDeviceToHost, st));
