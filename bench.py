@@ -43,13 +43,13 @@ FULL = {
     "cfg4": dict(desc="cfg4: continuous-energy pin cell, k-eigenvalue, 1e8 particles/gen, 1 inactive + 2 active generations, 100 energy bins", kw={}, ce=True),
 }
 HEADLINE = "cfg4"
-# (scheme, decomposition, stash) timed per workload; the first one of HEADLINE's list that is fastest becomes the headline
+# (scheme, decomposition, stash) timed per workload; the first one of HEADLINE's list is the headline (the fastest on cfg4, profiles/throughput_r02.md)
 VARIANTS = {
     "cfg0": [("stack", "fused", None), ("async", "fused", "index"), ("async", "hybrid", "shared")],
     "cfg1": [("stack", "fused", None), ("stack", "split", None), ("async", "fused", "index"), ("async", "hybrid", "shared"), ("async", "fused", "particle")],
     "cfg2": [("stack", "fused", None), ("async", "fused", "index"), ("async", "hybrid", "shared")],
     "cfg3": [("stack", "fused", None), ("async", "fused", "index"), ("async", "fused", "particle"), ("async", "hybrid", "shared")],
-    "cfg4": [("async", "fused", "index"), ("stack", "fused", None), ("async", "hybrid", "shared"), ("async", "split", "index"), ("stack", "split", None)],
+    "cfg4": [("stack", "fused", None), ("async", "fused", "index"), ("async", "hybrid", "shared"), ("async", "split", "index"), ("stack", "split", None)],
 }
 
 

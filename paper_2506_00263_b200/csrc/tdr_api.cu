@@ -38,7 +38,7 @@ struct tdr_problem {
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
   int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
-  int seg_per_launch = 0;                  // stack fused/hybrid: segments per particle per k_step launch; 0 = auto (3 multigroup, 8 continuous energy)
+  int seg_per_launch = 0;                  // stack fused/hybrid: segments per particle per k_step launch; 0 = auto (3 multigroup, 12 continuous energy)
   int force_spill = 0;                     // async stress option (tests): warps always believe another one is starved
   int seg_per_event = 0;                   // async fused: segments per step event before remapping; 0 = auto (2 multigroup, 5 continuous energy)
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
@@ -253,14 +253,17 @@ int tdr_init_problem(const tdr_geometry *g, const tdr_materials *m, const tdr_xs
     // X3: bucket = top bits (exponent + 7 mantissa bits) of E; hash[b] = largest i with grid[i] <= lower edge of b
     u64 blo, bhi; memcpy(&blo, &D.grid_lo, 8); memcpy(&bhi, &D.grid_hi, 8);
     D.hash_bmin = (u32)(blo >> 45); D.hash_n = (u32)(bhi >> 45) - D.hash_bmin + 1;
-    std::vector<u32> h(D.hash_n + 1);
+    std::vector<u32> h(D.hash_n + 1 + ((D.hash_n + 1) & 1u));            // (an even number of words: staged to shared memory as doubles)
     int i = 0;
     for (u32 b = 0; b <= D.hash_n; b++) {
       u64 eb = ((u64)(D.hash_bmin + b)) << 45; double edge; memcpy(&edge, &eb, 8);
       while (i + 1 < x->n_grid && x->energy[i + 1] <= edge) i++;
       h[b] = (u32)i;
     }
+    if (!h.empty()) h.back() = h[D.hash_n];
     UP(h.data(), h.size(), D.hash);
+    if (h.size() * 4 > 64 * 1024) { tdr_free_problem(p); return fail(TDR_EINVAL, "energy grid spans too many binades for the staged hash (%zu bytes)", h.size() * 4); }
+    D.mg = reinterpret_cast<const double *>(D.hash); D.mg_doubles = (int)(h.size() / 2);   // the block k_step, k_drain and k_async stage to shared memory (stage_mg)
   }
 #undef UP
   if (rc) { tdr_free_problem(p); return rc; }
@@ -424,7 +427,7 @@ static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, siz
   u64 *ctr = p->ctr;
   const DevRun *Rp = DEV ? p->run_dev : nullptr;
   auto cap = [&](int g) { return g < cap_blocks ? g : cap_blocks; };
-  const u32 spl = (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 8 : 3));
+  const u32 spl = (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 12 : 3));
   if (p->split == 1) {
     StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
     K.cnt = ctr + C_STACK0;
@@ -488,9 +491,11 @@ static int build_stack_graph(tdr_problem *p, size_t smem) {
 }
 
 // ---------------------------------------------------------------------------------- stack scheme, one generation
-static size_t smem_bytes(const tdr_problem *p) {      // dynamic shared memory = [MG table | private tally words]
+// dynamic shared memory = [staged table (multigroup rows | continuous energy: hash buckets + energy edges) | private tally words];
+// staged = false: a continuous-energy kernel that reads the block from global memory instead (stage_mg)
+static size_t smem_bytes(const tdr_problem *p, bool staged = true) {
   size_t priv = p->dp.n_bins <= PRIV_MAX_BINS ? (size_t)p->dp.n_bins * 16 : 0;
-  return (size_t)p->dp.mg_doubles * sizeof(double) + priv;
+  return ((p->ce && !staged) ? 0 : (size_t)p->dp.mg_doubles * sizeof(double)) + priv;
 }
 
 template <bool CE, bool EXT>
@@ -642,7 +647,7 @@ template <bool CE>
 static int run_pstash(tdr_problem *p, DevRun R) {
   cudaStream_t st = p->stream;
   const int threads = p->ps_threads;
-  const size_t smem = smem_bytes(p) + (threads / 32) * PsPool<CE>::bytes(p->pool_slots);
+  const size_t smem = smem_bytes(p, false) + (threads / 32) * PsPool<CE>::bytes(p->pool_slots);
   if (smem > 227 * 1024) return fail(TDR_EINVAL, "particle stash needs %zu bytes of shared memory per CTA (limit 227 KB)", smem);
   R.defer_death = 1; R.outstanding = p->ctr + C_PENDING; R.starved = p->ctr + C_STARVED; R.W = p->W;
   k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull);
@@ -681,7 +686,7 @@ static int run_cstash(tdr_problem *p, DevRun R) {
   const int threads = p->ps_threads <= CS_THREADS ? p->ps_threads : CS_THREADS;
   const int ns = p->pool_slots * (threads / 32);
   if (ns > 32768) return fail(TDR_EINVAL, "shared stash: more than 32768 slots per CTA");
-  const size_t smem = smem_bytes(p) + CsPool<CE>::bytes(ns);
+  const size_t smem = smem_bytes(p, false) + CsPool<CE>::bytes(ns);
   if (smem > 227 * 1024) return fail(TDR_EINVAL, "shared stash needs %zu bytes of shared memory per CTA (limit 227 KB)", smem);
   R.defer_death = 1; R.outstanding = p->ctr + C_PENDING; R.starved = p->ctr + C_STARVED; R.W = p->W;
   k_ps_init<<<64, 256, 0, st>>>(p->pm, R.outstanding, R.src_total, R.starved, p->force_spill ? (1ull << 40) : 0ull);

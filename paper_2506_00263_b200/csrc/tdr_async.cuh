@@ -218,8 +218,8 @@ __global__ void __launch_bounds__(TDR_ASYNC_MAXT, 1) k_async(DevProb P0, DevOut 
   const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
-  const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const double *mg = stage_mg(P, smem, true);
+  const TallyPriv tp = stage_priv(P, smem, mg, true);
   acc_init(&acc);
   WarpCtx w;
   w.lane = threadIdx.x & 31; w.gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w.A = A; w.err = O.err;

@@ -130,9 +130,9 @@ __global__ void __launch_bounds__(CS_THREADS, CS_MINB) k_cstash(DevProb P0, DevO
   __shared__ BlockAcc acc;
   __shared__ CsCtl ctl;
   const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const TallyPriv tp = stage_priv(P, smem, mg);
   CsPool<CE> pl;
-  pl.bind((char *)(smem + P.mg_doubles) + 16 * tp.n, NS);
+  pl.bind((char *)(smem + staged_doubles(P, false)) + 16 * tp.n, NS);
   const u32 lane = threadIdx.x & 31, wid = threadIdx.x >> 5, nw = blockDim.x >> 5, cap = nw * 32;
   for (u32 i = threadIdx.x; i < (u32)NS; i += blockDim.x) { pl.ring[CE_BIRTH][i] = (unsigned short)i; pl.w[i] = CS_FRESH; }
   if (threadIdx.x == 0) {

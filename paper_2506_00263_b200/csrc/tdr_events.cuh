@@ -99,9 +99,9 @@ __device__ __forceinline__ int cell_material(const PT &P, const Part &p, int &un
   return P.univ_mat[univ * (TDR_MAX_RINGS + 1) + p.ring];
 }
 
-__device__ __forceinline__ int grid_index(const DevProb &P, double El) {   // X3 hashed search == X2 index
+__device__ __forceinline__ int grid_index(const DevProb &P, const u32 *hash, double El) {   // X3 hashed search == X2 index; hash: the staged buckets
   u32 b = (u32)((u64)__double_as_longlong(El) >> 45) - P.hash_bmin;
-  u32 lo = P.hash[b], hi = P.hash[b + 1] + 1;       // grid[lo] <= El (or lo == 0), answer in [lo, hi)
+  u32 lo = hash[b], hi = hash[b + 1] + 1;           // grid[lo] <= El (or lo == 0), answer in [lo, hi)
   if (hi > (u32)P.n_grid) hi = (u32)P.n_grid;
   while (hi - lo > 1) {
     u32 mid = lo + ((hi - lo) >> 1);
@@ -121,7 +121,7 @@ __device__ __forceinline__ void ev_lookup(const PT &P, const double *mg, const P
     St = row[0]; nsf = row[3]; gi = 0; f = 0.0;
   } else {
     double El = p.E; if (El < P.grid_lo) El = P.grid_lo; if (El > P.grid_hi) El = P.grid_hi;
-    gi = grid_index(P, El);
+    gi = grid_index(P, reinterpret_cast<const u32 *>(mg), El);
     double e0 = P.grid[gi], e1 = P.grid[gi + 1];
     f = (El - e0) / (e1 - e0);
     St = 0.0; nsf = 0.0;

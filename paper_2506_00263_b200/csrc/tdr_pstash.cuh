@@ -77,14 +77,14 @@ __global__ void __launch_bounds__(PS_THREADS, PS_MINB) k_pstash(DevProb P0, DevO
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const TallyPriv tp = stage_priv(P, smem, mg);
   acc_init(&acc);
   PsWarp w;
   w.lane = threadIdx.x & 31; w.gw = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); w.A = A; w.err = O.err;
   w.open_id = NOLINK; w.open_count = 0; w.n_spill = 0; w.n_fetch = 0;
   const u32 lane = w.lane;
   PsPool<CE> pl;
-  pl.bind((char *)(smem + P.mg_doubles) + 16 * tp.n + (threadIdx.x >> 5) * PsPool<CE>::bytes(NS), NS);
+  pl.bind((char *)(smem + staged_doubles(P, false)) + 16 * tp.n + (threadIdx.x >> 5) * PsPool<CE>::bytes(NS), NS);
   PsRing mq, cq, bq;
   mq.buf = pl.rings(); cq.buf = mq.buf + PS_RING; bq.buf = cq.buf + PS_RING;
   mq.head = mq.count = cq.head = cq.count = 0; bq.head = 0; bq.count = (u32)NS;

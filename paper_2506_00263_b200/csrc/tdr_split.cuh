@@ -16,7 +16,7 @@ __global__ void __launch_bounds__(256) k_event(DevProb P0, DevOut O, DevRun Rv, 
   __shared__ BlockAcc acc;
   TDR_BIND_RUN(DEV, Rv, Rp)
   const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const TallyPriv tp = stage_priv(P, smem, mg);
   acc_init(&acc);
   if (blockIdx.x == 0 && threadIdx.x == 0 && zero_ev >= 0) K.cnt[zero_ev] = 0;   // the stack the previous kernel drained
   const u64 n_in = K.cnt[EV];
@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(256) k_collide(DevProb P0, DevOut O, DevRun Rv
   __shared__ BlockAcc acc;
   TDR_BIND_RUN(DEV, Rv, Rp)
   const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const TallyPriv tp = stage_priv(P, smem, mg);
   acc_init(&acc);
   const u64 n_in = *ccount;
   i64 accP = 0, accPc = 0;

@@ -82,13 +82,22 @@ __device__ __forceinline__ bool make_work(const DevProb &P, const double *mg, co
   return reborn;
 }
 
-__device__ __forceinline__ const double *stage_mg(const DevProb &P, double *smem) {
-  if (P.G == 0) return nullptr;
+// The table every lookup of the run reads, staged to shared memory by each CTA: the multigroup rows (X1), or, in continuous
+// energy, the hash buckets of the energy grid (X3; BASELINE.json north_star: "hashed binary search staged through shared
+// memory") — the events receive the block as `mg` either way.
+// stage_ce = false: a continuous-energy kernel that would not win the copy back (one event per thread and launch, or a
+// stash that needs the shared memory as L1: measured, profiles/ncu_r02.md) reads the same block from global memory.
+__device__ __forceinline__ const double *stage_mg(const DevProb &P, double *smem, bool stage_ce = false) {
+  if (P.mg_doubles == 0) return nullptr;
+  if (P.G == 0 && !stage_ce) return P.mg;
   for (int i = threadIdx.x; i < P.mg_doubles; i += blockDim.x) smem[i] = P.mg[i];
   return smem;
 }
 // dynamic shared memory = [MG table | private tally words]; host side: smem_bytes()
-__device__ __forceinline__ TallyPriv stage_priv(const DevProb &P, double *smem) { return priv_init(P, smem + P.mg_doubles); }
+__device__ __forceinline__ int staged_doubles(const DevProb &P, bool stage_ce) { return (P.G == 0 && !stage_ce) ? 0 : P.mg_doubles; }
+__device__ __forceinline__ TallyPriv stage_priv(const DevProb &P, double *smem, const double *mg, bool stage_ce = false) {
+  return priv_init(P, smem + staged_doubles(P, stage_ce));
+}
 
 // ---------------------------------------------------------------------------------- A1 SOURCE: fill slots [0, n)
 template <bool CE>
@@ -153,8 +162,8 @@ __global__ void __launch_bounds__(256, 2) k_step(DevProb P0, DevOut O, DevRun Rv
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
   TDR_BIND_RUN(DEV, Rv, Rp)
-  const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const double *mg = stage_mg(P, smem, true);
+  const TallyPriv tp = stage_priv(P, smem, mg, true);
   acc_init(&acc);
   const u64 n_in = *count_in;
   i64 accP = 0, accPc = 0;
@@ -209,8 +218,8 @@ __global__ void __launch_bounds__(256) k_drain(DevProb P0, DevOut O, DevRun R, S
   const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   extern __shared__ double smem[];
   __shared__ BlockAcc acc;
-  const double *mg = stage_mg(P, smem);
-  const TallyPriv tp = stage_priv(P, smem);
+  const double *mg = stage_mg(P, smem, true);
+  const TallyPriv tp = stage_priv(P, smem, mg, true);
   acc_init(&acc);
   const u64 n_in = *count_in;
   i64 accP = 0, accPc = 0;

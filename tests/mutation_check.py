@@ -55,7 +55,7 @@ MUTANTS = [
     ("mesh_dec", "if (q->mx > 0) q->mx -= 1; } }", "if (q->mx > 0) q->mx -= 0; } }", "T7 mesh index -x"),
     ("mesh_dist_z", "if (dmz < ds) ds = dmz;", "", "T3 mesh-plane candidate (z) dropped"),
     ("mesh_dist_y", "if (dmy < ds) ds = dmy;", "", "T3 mesh-plane candidate (y) dropped"),
-    ("mesh_bin_index", "bin = ((((size_t)q->mz * p->mesh_n[1] + q->my) * p->mesh_n[0]) + q->mx) * p->n_e + e;", "bin = ((((size_t)q->mz * p->mesh_n[1] + q->my) * p->mesh_n[0]) + q->mx) * p->n_e;", "T5 energy offset of the bin"),
+    ("mesh_bin_index", "+ q->mx) * p->n_e + e;   /* TD4", "+ q->mx) * p->n_e;   /* TD4", "T5 energy offset of the bin"),
     ("plane_dist_neg", "if (c < 0.0) return (lo - x) / c;", "if (c < 0.0) return (x - lo) / c;", "G3 plane distance for c < 0"),
     ("cyl_inside_root", "d = (-b + sqrt(disc)) / a;", "d = (-b - sqrt(disc)) / a;", "G4 leaving root"),
     ("cyl_c_term", "double c = (X * X + Y * Y) - R * R;", "double c = (X * X + Y * Y) - R;", "G4 constant term"),
@@ -63,7 +63,7 @@ MUTANTS = [
     ("leak_face", "else { alive = 0; c->leak[1] += 1; } } else { q->ix += 1;", "else { alive = 0; c->leak[0] += 1; } } else { q->ix += 1;", "G7 leak booked on the wrong face"),
     ("tie_rule", "int collide = dcoll < ds;", "int collide = dcoll <= ds;", "G5 tie rule (EQUIVALENT in practice: ties have measure zero)"),
     ("advance", "q->x = q->x + d * u0;", "q->x = q->x + d * v0;", "G6 advance"),
-    ("flux_score", "fixp(p, d), &c->flux[bin])", "fixp(p, dcoll), &c->flux[bin])", "T5 scores the collision distance, not the flight"),
+    ("flux_score", "const double wd = p->implicit ? q->wgt * d : d;", "const double wd = p->implicit ? q->wgt * d : dcoll;", "T5 scores the collision distance, not the flight"),
     ("pc_score", "c->Pc += fixp(p, nsf / St);", "c->Pc += fixp(p, nsf);", "T6 collision estimator of k"),
     ("p_score", "c->P += fixp(p, d * nsf);", "c->P += fixp(p, d * St);", "T5 track-length estimator of k"),
     ("mg_select", "if (r < sst) kind = 0; else if (r < sst + p->sig_c[mat * p->G + q->g]) kind = 1; else kind = 2;", "if (r < sst) kind = 0; else if (r < p->sig_c[mat * p->G + q->g]) kind = 1; else kind = 2;", "T6 MG capture threshold"),
@@ -74,9 +74,9 @@ MUTANTS = [
     ("child_tag", "s.id = orc_derive_id(seed, q->id, gen, seg, (uint32_t)k);", "s.id = orc_derive_id(seed, q->id, gen, seg, 0u);", "R4 children share one id"),
     ("child_depth", "s.depth = (uint8_t)(c->kmode ? 0 : q->depth + 1);", "s.depth = (uint8_t)(c->kmode ? 0 : q->depth);", "D1 depth never grows (cap never reached)"),
     ("secondaries_lost", "while (!c.err && c.stack.n > 0) {", "while (0) {", "D1 secondaries never run"),
-    ("popctrl_round", "int m = (int)floor(pr + orc_draw(seed, b->id, g + 1, 0, PUR_POPCTRL, 0));", "int m = (int)floor(pr + 0.5);", "D2 deterministic rounding in population control"),
-    ("popctrl_tag", "cp.id = orc_derive_id(seed, b->id, g + 1, 0, 2048u + (uint32_t)r);", "cp.id = orc_derive_id(seed, b->id, g + 1, 0, 2048u);", "R4 copies of a site share one id"),
-    ("k_formula", "double k = ((double)(int64_t)o.P * (1.0 / p->scale)) / (double)n_src;", "double k = ((double)(int64_t)o.Pc * (1.0 / p->scale)) / (double)n;", "D2 k from the wrong tally and divisor (EQUIVALENT within statistics: both estimators are unbiased)"),
+    ("popctrl_round", "int m = (int)floor(pr + orc_draw(p->kseed, b->id, gen_next, 0, PUR_POPCTRL, 0));", "int m = (int)floor(pr + 0.5);", "D2 deterministic rounding in population control"),
+    ("popctrl_tag", "cp.id = orc_derive_id(p->kseed, b->id, gen_next, 0, 2048u + (uint32_t)r);", "cp.id = orc_derive_id(p->kseed, b->id, gen_next, 0, 2048u);", "R4 copies of a site share one id"),
+    ("k_formula", "double k = ((double)sums[0] * (1.0 / p->scale)) / (double)sums[2];", "double k = ((double)sums[1] * (1.0 / p->scale)) / (double)sums[2];", "D2 k from the collision estimator (EQUIVALENT within statistics: both estimators are unbiased)"),
     ("watt_cos2", "cos2 = (v1 * v1) / s; break; }", "cos2 = (v1 * v1); break; }", "B3 Watt cos^2"),
     ("watt_shift", "return (W + aab / 4.0) + (2.0 * x2 - 1.0) * sqrt(aab * W);", "return (W + aab / 2.0) + (2.0 * x2 - 1.0) * sqrt(aab * W);", "B3 Watt shift term"),
     ("iso_w", "out[0] = v1 * t; out[1] = v2 * t; out[2] = 1.0 - 2.0 * s;", "out[0] = v1 * t; out[1] = v2 * t; out[2] = 1.0 - s;", "B2 Marsaglia w"),
