@@ -143,7 +143,7 @@ def test_stack_remap_loop_runs_to_extinction_without_the_tail_drain(decomp, devi
     for p in (W.cfg1(n=30011, n_inactive=1, n_active=2), W.cfg4(n=20011, n_inactive=1, n_active=1)):
         o, g, d = run_both(p, scheme="stack", decomposition=decomp, drain_below=0, device_loop=device_loop)
         assert_same(o, g, f"{p.name}/stack/{decomp}/drain_below=0/device_loop={device_loop}")
-        assert d["iterations"] > 30, d
+        assert d["iterations"] > 15, d                     # (cfg4 follows a particle for 12 segments per launch)
 
 
 @pytest.mark.parametrize("decomp", ["fused", "hybrid", "split"])
