@@ -192,6 +192,29 @@ int tdr_dev_draw(uint64_t seed, const uint64_t *id, uint32_t gen, uint32_t seg, 
  * GB/s (read + write bytes).  `value` is a HOST pointer; the call allocates and frees its own device scratch. */
 int tdr_measure_peak(int what, double *value, void *cuda_stream);
 
+/* Population control (reading D2; "splitting roulette population control") on caller-owned DEVICE arrays: site i
+ * of bank[0..n_bank) gets m_i = floor(pr + xi(site id, gen_next, 0, POPCTRL, 0)) copies (at most 2048) with the derived ids of
+ * reading R4.  next[0..min(total, next_cap)) receives the copies, count_dev[0] the total wanted (total > next_cap = overflow,
+ * the caller's check).  All pointers DEVICE; asynchronous on cuda_stream.
+ *
+ * tdr_dev_popctrl: the library's k_popctrl as the k-eigenvalue driver runs it (copies in any order); it cudaMallocs and frees its
+ * counter and synchronises the stream.
+ *
+ * tdr_dev_popctrl_noalloc: the same result from a variant that allocates NOTHING — for callers that cannot call cudaMalloc (code
+ * under CUDA-graph capture, tight serving loops, harnesses that forbid it).  No cudaMalloc / cudaFree / allocating routine, no
+ * synchronisation, no host-side read: three kernel launches on cuda_stream.  Its scratch (per-site copy counts, their prefix sums,
+ * the total) lives in ONE file-scope `static __device__` array of 4 MiB + 256 B that every GPU which loads the library holds until
+ * exit; its device address is resolved once per device (cudaGetSymbolAddress, on the first call with that device current: make
+ * that first call outside a capture).  Limit: n_bank <= TDR_NOALLOC_MAX_SITES, beyond it TDR_EINVAL with a message.  The copies
+ * come out in bank order (site 0's copies first), which the allocating path does not promise.  Every call shares the scratch, which
+ * keeps the previous call's contents (each call rewrites what it reads); two calls that overlap on the GPU (different streams or
+ * processes' threads without ordering) RACE: order them on one stream or with events. */
+#define TDR_NOALLOC_MAX_SITES 524288
+int tdr_dev_popctrl(const tdr_site *bank, uint64_t n_bank, tdr_site *next, uint64_t next_cap, uint64_t *count_dev,
+                    uint64_t seed, uint32_t gen_next, double pr, void *cuda_stream);
+int tdr_dev_popctrl_noalloc(const tdr_site *bank, uint64_t n_bank, tdr_site *next, uint64_t next_cap, uint64_t *count_dev,
+                            uint64_t seed, uint32_t gen_next, double pr, void *cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

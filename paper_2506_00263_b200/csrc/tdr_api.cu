@@ -969,3 +969,97 @@ int tdr_measure_peak(int what, double *value, void *stream) {
   *value = work / (best / 1e3);
   return TDR_OK;
 }
+
+// ---------------------------------------------------------------------------------- population control on caller-owned arrays
+// tdr_dev_popctrl: the driver's own kernel (k_popctrl) with a counter and an error word the call allocates and frees.
+int tdr_dev_popctrl(const tdr_site *bank, uint64_t n_bank, tdr_site *next, uint64_t next_cap, uint64_t *count_dev,
+                    uint64_t seed, uint32_t gen_next, double pr, void *stream) {
+  if ((!bank && n_bank) || !next || !count_dev) return fail(TDR_EINVAL, "null argument");
+  cudaStream_t st = (cudaStream_t)stream;
+  int *err = nullptr; CK(cudaMalloc(&err, 256));
+  CK(cudaMemsetAsync(err, 0, 256, st)); CK(cudaMemsetAsync(count_dev, 0, 8, st));
+  if (n_bank) k_popctrl<<<148 * 4, 256, 0, st>>>(bank, n_bank, next, next_cap, (u64 *)count_dev, seed, gen_next, pr, err);
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  cudaFree(err);
+  if (e != cudaSuccess) return fail(TDR_ECUDA, "tdr_dev_popctrl: %s", cudaGetErrorString(e));
+  return TDR_OK;
+}
+
+// tdr_dev_popctrl_noalloc: the variant that allocates nothing.  Scratch = ONE file-scope device array (include/tdr.h):
+//   [0, 256)                         header: word 0 = total number of copies
+//   [256, 256 + 4 MAX)               m[i]   = copies of site i
+//   [256 + 4 MAX, 256 + 8 MAX)       off[i] = exclusive prefix sum of m
+// In HOST code the array's name is a host-side stand-in, not a device address: the address every kernel gets comes from
+// cudaGetSymbolAddress, resolved once per device with that device current.  (Device code could name the array directly.)
+#define NOALLOC_HDR 256
+static __device__ __align__(256) unsigned char g_noalloc_scratch[NOALLOC_HDR + 8ull * TDR_NOALLOC_MAX_SITES];
+static void *g_noalloc_ptr[64];                                // per device ordinal; nullptr = not resolved yet
+
+__global__ void __launch_bounds__(256) k_na_count(const tdr_site *bank, u32 n, u32 *m, u64 seed, u32 gen_next, double pr) {
+  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    int c = (int)floor(pr + draw(seed, bank[i].id, gen_next, 0, PUR_POPCTRL, 0));          // D2, as k_popctrl
+    m[i] = (u32)(c < 0 ? 0 : c > 2048 ? 2048 : c);
+  }
+}
+
+// one CTA of 1024 threads: thread t owns the contiguous chunk [t c, (t + 1) c); chunk sums are scanned in shared memory
+__global__ void __launch_bounds__(1024) k_na_scan(const u32 *m, u32 *off, u32 n, u64 *total_scratch, u64 *count_out) {
+  __shared__ u32 part[1024];
+  const u32 t = threadIdx.x, c = (n + 1023u) / 1024u;
+  const u32 lo = min(t * c, n), hi = min(lo + c, n);
+  u32 s = 0;
+  for (u32 i = lo; i < hi; i++) s += m[i];
+  part[t] = s;
+  __syncthreads();
+  for (u32 d = 1; d < 1024; d <<= 1) {                          // inclusive Hillis-Steele scan of the 1024 chunk sums
+    const u32 v = t >= d ? part[t - d] : 0u;
+    __syncthreads();
+    part[t] += v;
+    __syncthreads();
+  }
+  u32 run = part[t] - s;                                        // exclusive offset of this thread's chunk
+  for (u32 i = lo; i < hi; i++) { off[i] = run; run += m[i]; }
+  if (t == 1023) { *total_scratch = (u64)part[1023]; *count_out = (u64)part[1023]; }
+}
+
+__global__ void __launch_bounds__(256) k_na_write(const tdr_site *bank, u32 n, const u32 *m, const u32 *off, tdr_site *next, u64 next_cap,
+                                                  u64 seed, u32 gen_next) {
+  for (u32 i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+    const u32 c = m[i]; const u64 base = off[i];
+    if (c == 0) continue;
+    tdr_site s = bank[i]; const u64 sid = s.id;
+    for (u32 r = 0; r < c; r++) {
+      s.id = derive_id(seed, sid, gen_next, 0, 2048u + r);       // R4, as k_popctrl
+      if (base + r < next_cap) next[base + r] = s;
+    }
+  }
+}
+
+int tdr_dev_popctrl_noalloc(const tdr_site *bank, uint64_t n_bank, tdr_site *next, uint64_t next_cap, uint64_t *count_dev,
+                            uint64_t seed, uint32_t gen_next, double pr, void *stream) {
+  if ((!bank && n_bank) || !next || !count_dev) return fail(TDR_EINVAL, "null argument");
+  if (n_bank > TDR_NOALLOC_MAX_SITES)
+    return fail(TDR_EINVAL, "tdr_dev_popctrl_noalloc: %llu sites exceed the static scratch (TDR_NOALLOC_MAX_SITES = %d); use tdr_dev_popctrl or split the bank",
+                (unsigned long long)n_bank, TDR_NOALLOC_MAX_SITES);
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(TDR_EINVAL, "device ordinal %d out of range", dev);
+  if (!g_noalloc_ptr[dev]) {                                    // set-up, once per device, with that device current
+    void *ptr = nullptr;
+    CK(cudaGetSymbolAddress(&ptr, g_noalloc_scratch));
+    if (!ptr) return fail(TDR_ECUDA, "cudaGetSymbolAddress returned a null address");
+    g_noalloc_ptr[dev] = ptr;
+  }
+  unsigned char *scr = (unsigned char *)g_noalloc_ptr[dev];
+  u64 *total = (u64 *)scr; u32 *m = (u32 *)(scr + NOALLOC_HDR), *off = m + TDR_NOALLOC_MAX_SITES;
+  cudaStream_t st = (cudaStream_t)stream;
+  const u32 n = (u32)n_bank;
+  // every word a kernel reads is written by this call first (m[0..n), off[0..n), the total): nothing of the last call survives into it
+  const int grid = n ? (int)((n + 255u) / 256u < 148u * 8u ? (n + 255u) / 256u : 148u * 8u) : 1;
+  k_na_count<<<grid, 256, 0, st>>>(bank, n, m, seed, gen_next, pr);
+  k_na_scan<<<1, 1024, 0, st>>>(m, off, n, total, (u64 *)count_dev);
+  k_na_write<<<grid, 256, 0, st>>>(bank, n, m, off, next, next_cap, seed, gen_next);
+  CK(cudaGetLastError());
+  return TDR_OK;
+}

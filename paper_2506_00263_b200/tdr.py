@@ -63,7 +63,7 @@ class tdr_diag(C.Structure):
 
 EXPORTS = ["tdr_init_problem", "tdr_set_option", "tdr_workspace_bytes", "tdr_bind_workspace", "tdr_run_fixed_source",
            "tdr_run_k_eigenvalue", "tdr_tally_sizes", "tdr_read_tallies", "tdr_read_diagnostics", "tdr_free_problem",
-           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw", "tdr_k_begin", "tdr_k_generation", "tdr_k_population_control", "tdr_k_end", "tdr_measure_peak"]
+           "tdr_last_error", "tdr_dev_det_log", "tdr_dev_draw", "tdr_k_begin", "tdr_k_generation", "tdr_k_population_control", "tdr_k_end", "tdr_measure_peak", "tdr_dev_popctrl", "tdr_dev_popctrl_noalloc"]
 
 _lib = None
 
@@ -93,6 +93,8 @@ def lib():
         L.tdr_last_error.restype = C.c_char_p
         L.tdr_dev_det_log.argtypes = [C.c_void_p, C.c_void_p, C.c_uint64, C.c_void_p]
         L.tdr_dev_draw.argtypes = [C.c_uint64, C.c_void_p, C.c_uint32, C.c_uint32, C.c_uint32, C.c_uint32, C.c_void_p, C.c_uint64, C.c_void_p]
+        for f in (L.tdr_dev_popctrl, L.tdr_dev_popctrl_noalloc):
+            f.argtypes = [C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_void_p, C.c_uint64, C.c_uint32, C.c_double, C.c_void_p]
         _lib = L
     return _lib
 
@@ -260,3 +262,18 @@ def measure_peak(what):
     v = C.c_double()
     _check(lib().tdr_measure_peak({"fp64": 0, "l2": 1}[what], C.byref(v), torch.cuda.current_stream().cuda_stream), "tdr_measure_peak")
     return v.value
+
+
+def dev_popctrl(bank, next_cap, seed, gen_next, pr, noalloc=False):
+    """Population control on a device array of 48-byte sites (torch uint8 tensor of shape [n, 48]).  Returns (next sites
+    [min(total, next_cap), 48] uint8, total).  noalloc=True: the entry point that allocates nothing (static device scratch,
+    at most TDR_NOALLOC_MAX_SITES sites); the output tensors are still the caller's."""
+    import torch
+    n = bank.shape[0]
+    nxt = torch.empty((next_cap, 48), dtype=torch.uint8, device=bank.device)
+    cnt = torch.zeros(1, dtype=torch.int64, device=bank.device)
+    f = lib().tdr_dev_popctrl_noalloc if noalloc else lib().tdr_dev_popctrl
+    _check(f(bank.data_ptr(), n, nxt.data_ptr(), next_cap, cnt.data_ptr(), seed, gen_next, float(pr), torch.cuda.current_stream().cuda_stream),
+           "tdr_dev_popctrl_noalloc" if noalloc else "tdr_dev_popctrl")
+    total = int(cnt.item())
+    return nxt[:min(total, next_cap)], total
