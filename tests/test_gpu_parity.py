@@ -402,3 +402,25 @@ def test_general_cells_full_generation_and_refusals():
     from oracle import orc
     with pytest.raises(RuntimeError, match="-5"):
         orc.run(bad)
+
+
+# ------------------------------------------------------------------ BASELINE's full per-generation sizes
+@pytest.mark.parametrize("scheme,decomp,stash", [("stack", "fused", None), ("async", "fused", "index"), ("async", "hybrid", "shared")])
+def test_ten_million_particles_per_generation(scheme, decomp, stash):
+    """cfg2 at its full size per generation (1e7) and cfg4 at 1e7 (a tenth of its 1e8; the oracle needs minutes for more), in the
+    launch configuration bench.py times (no history records): everything that is unique and has a size independent of N —
+    totals with the order-independent history digest, all tallies, leak, per-generation N / M / P / Pc, k."""
+    from paper_2506_00263_b200 import tdr
+    from tests.parity import oracle_result
+    for p in (W.cfg2(n=10000000, n_inactive=1, n_active=1), W.cfg4(n=10000000, n_inactive=1, n_active=1)):
+        o = oracle_result(p)
+        P = tdr.Problem(p, scheme=scheme, decomposition=decomp, keep_history=0, **({"stash": stash} if stash else {}))
+        try:
+            P.run_k_eigenvalue(p.n_particles, p.n_inactive, p.n_active, p.seed)
+            g = P.read_tallies(history=False, bank=False)
+        finally:
+            P.close()
+        assert o["totals"] == g["totals"], (p.name, scheme)
+        for k in ("flux", "coll", "leak", "gen_n", "gen_m", "gen_p", "gen_pc"):
+            assert np.array_equal(o[k], g[k]), (p.name, scheme, k)
+        assert np.allclose(o["gen_k"], g["gen_k"], rtol=1e-12, atol=0)
