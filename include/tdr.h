@@ -143,6 +143,7 @@ int tdr_init_problem(const tdr_geometry *, const tdr_materials *, const tdr_xs_t
  * counter read-back); "blocks_per_sm"; "keep_history" = 0|1; "time_kernels" = 0|1; "idle_timeout_s" (async watchdog);
  * "seg_per_event" (async fused: segments per step event); "seg_per_launch", "drain_below" (stack); "lockstep",
  * "async_threads" (async); "id_offset" (fixed source: ids id_offset .. id_offset+n-1, for sharding one source over several GPUs);
+ * "step_lockstep" = -1|0|1 (stack: CTA-wide lockstep of the segments inside k_step; -1 = auto: multigroup only);
  * "device_loop" = 1|0 (stack: the remap loop runs as a CUDA-graph WHILE node without the host | host-driven batches of sync_every);
  * "stash" = auto|index|particle|shared, "pool_slots", "ps_threads" (async: which stash).
  * decomposition = fused (monolithic step) | split (five events) | hybrid (step + collide). */

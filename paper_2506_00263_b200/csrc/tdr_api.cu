@@ -38,7 +38,7 @@ struct tdr_problem {
   int keep_history = -1;                   // -1 auto (n <= 2e6)
   int time_kernels = 0;
   int lockstep = 1, async_threads = 512;   // async scheme: CTA-wide lockstep phase; threads per CTA (256 or 512)
-  int seg_per_launch = 0;                  // stack fused/hybrid: segments per particle per k_step launch; 0 = auto (3 multigroup, 12 continuous energy)
+  int seg_per_launch = 0;                  // stack fused/hybrid: segments per particle per k_step launch; 0 = auto (6 multigroup, 12 continuous energy)
   int force_spill = 0;                     // async stress option (tests): warps always believe another one is starved
   int seg_per_event = 0;                   // async fused: segments per step event before remapping; 0 = auto (2 multigroup, 5 continuous energy)
   int slots_per_warp = 128;                // async scheme: window slots a warp may claim for itself
@@ -71,6 +71,7 @@ struct tdr_problem {
   // stack scheme, device-driven remap loop: a CUDA graph with one WHILE node (built per run), its capture stream, and the
   // DevRun the graph's kernels read
   int device_loop = 1;
+  int step_lockstep = -1;                  // stack fused/hybrid: the CTA's warps run the segments of a k_step tile in lockstep; -1 = auto (multigroup only)
   cudaGraph_t sg_graph = nullptr; cudaGraphExec_t sg_exec = nullptr; cudaStream_t sg_capture = nullptr; int sg_per_pass = 0;
   DevRun *run_dev = nullptr;
 };
@@ -300,6 +301,7 @@ int tdr_set_option(tdr_problem *p, const char *key, const char *value) {
   else if (k == "bank_cap") p->bank_cap_opt = strtoull(value, nullptr, 10);
   else if (k == "arena_links") p->arena_links_opt = strtoull(value, nullptr, 10);
   else if (k == "device_loop") p->device_loop = atoi(value) != 0;
+  else if (k == "step_lockstep") { int n = atoi(value); if (n < -1 || n > 1) return fail(TDR_EINVAL, "step_lockstep: -1 (auto), 0 or 1"); p->step_lockstep = n; }
   else if (k == "sync_every") { int n = atoi(value); if (n < 1 || n > 1024) return fail(TDR_EINVAL, "sync_every in [1,1024]"); p->sync_every = n; }
   else return fail(TDR_EINVAL, "unknown option %s", key);
   return TDR_OK;
@@ -427,7 +429,8 @@ static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, siz
   u64 *ctr = p->ctr;
   const DevRun *Rp = DEV ? p->run_dev : nullptr;
   auto cap = [&](int g) { return g < cap_blocks ? g : cap_blocks; };
-  const u32 spl = (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 12 : 3));
+  const u32 spl = (u32)(p->seg_per_launch ? p->seg_per_launch : (CE ? 12 : 6));
+  const int sls = p->step_lockstep < 0 ? !CE : p->step_lockstep;       // segment lockstep inside k_step: multigroup only by default
   if (p->split == 1) {
     StackSet K; for (int e = 0; e < EV_COUNT; e++) K.s[e] = p->stacks[e];
     K.cnt = ctr + C_STACK0;
@@ -441,23 +444,23 @@ static int remap_iteration(tdr_problem *p, const DevRun &R, cudaStream_t st, siz
   // fused / hybrid: two index stacks, three rotating counters (in, out, the one to clear)
   if (DEV) {                                       // the kernels derive the iteration's pointers themselves: bases only
     if (p->split == 2) {
-      k_step<CE, true, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, p->stacks[2], nullptr, nullptr, spl);
+      k_step<CE, true, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, p->stacks[2], nullptr, nullptr, spl, sls);
       k_collide<CE, true, EXT><<<G.coll, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], ctr, p->stacks[0], reinterpret_cast<u64 *>(p->stacks[1]));
       return 2;
     }
-    k_step<CE, false, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, nullptr, nullptr, nullptr, spl);
+    k_step<CE, false, true, EXT><<<G.step, 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[0], ctr, p->stacks[1], nullptr, nullptr, nullptr, nullptr, nullptr, spl, sls);
     return 1;
   }
   const int in = (int)(it % 3), out = (int)((it + 1) % 3), zr = (int)((it + 2) % 3);
   if (p->split == 2) {
     u64 *cc = ctr + C_STACK0 + 3 + (it & 1), *cz = ctr + C_STACK0 + 3 + ((it + 1) & 1);      // collide-stack counters
     k_step<CE, true, DEV, EXT><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                          p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, spl);
+                                                          p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, p->stacks[2], cc, cz, spl, sls);
     k_collide<CE, DEV, EXT><<<cap(G.coll), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[2], cc, p->stacks[(it + 1) & 1], ctr + C_STACK0 + out);
     return 2;
   }
   k_step<CE, false, DEV, EXT><<<cap(G.step), 256, smem, st>>>(p->dp, p->out, R, Rp, p->soa, p->stacks[it & 1], ctr + C_STACK0 + in,
-                                                         p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, spl);
+                                                         p->stacks[(it + 1) & 1], ctr + C_STACK0 + out, ctr + C_STACK0 + zr, nullptr, nullptr, nullptr, spl, sls);
   return 1;
 }
 

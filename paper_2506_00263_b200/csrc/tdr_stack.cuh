@@ -144,7 +144,7 @@ __global__ void __launch_bounds__(256) k_source(DevProb P, DevOut O, DevRun R, S
 template <bool CE, bool HYBRID, bool DEV, bool EXT>
 __global__ void __launch_bounds__(256, 2) k_step(DevProb P0, DevOut O, DevRun Rv, const DevRun *Rp, Soa S0, const u32 *stack_in, const u64 *count_in,
                                               u32 *stack_out, u64 *count_out, u64 *count_zero,
-                                              u32 *cstack, u64 *ccount, u64 *ccount_zero, u32 seg_per_launch) {
+                                              u32 *cstack, u64 *ccount, u64 *ccount_zero, u32 seg_per_launch, int sync_seg) {
   const ProbX<EXT> &P = static_cast<const ProbX<EXT> &>(P0);
   const SoaX<EXT> &S = static_cast<const SoaX<EXT> &>(S0);
   if (DEV) {
@@ -173,6 +173,9 @@ __global__ void __launch_bounds__(256, 2) k_step(DevProb P0, DevOut O, DevRun Rv
     bool valid = i < n_in;
     Part p; u32 slot = 0;
     if (valid) { slot = stack_in[i]; load_part<CE>(S, slot, p); }
+    // sync_seg: the CTA's warps also start every SEGMENT of the tile together and leave the loop together (the vote below), so the
+    // lines one warp fetches serve the others for the whole tile, as in the persistent kernel's lockstep (+7 ... +19 % in
+    // multigroup, -5 ... -7 % in continuous energy where the cross-section gathers make segments uneven: profiles/ncu_r02.md)
     // up to seg_per_launch segments per particle in registers before it is pushed again ("history-length truncation",
     // PAPER.md:119, with a length > 1): fewer launches and state round trips; a lane whose particle died idles
     bool alive = valid, to_collide = false;
@@ -195,7 +198,7 @@ __global__ void __launch_bounds__(256, 2) k_step(DevProb P0, DevOut O, DevRun Rv
         else alive = ev_surface(P, R, &acc, p, flags);
       }
       if (!HYBRID) push_children(O, R, &acc, p, nch, csrc);
-      if (!__any_sync(FULL, alive)) break;
+      if (sync_seg ? !__syncthreads_or(alive) : !__any_sync(FULL, alive)) break;
     }
     if (make_work<CE>(P, mg, R, &acc, p, valid && !alive && !to_collide)) alive = true;
     if (alive) store_part<CE>(S, slot, p);
